@@ -1,0 +1,123 @@
+/*
+ * ts_b200.h -- C ABI of libts_b200.so: the Trotter-Suzuki time step of arXiv:1305.0036 on one B200 (sm_100a).
+ *
+ * "P:<n>" = line n of the paper text; "A<n>" = a reading listed in DESIGN.md.
+ *
+ * What the library computes: for the spin-1/2 Hamiltonian of eq. 1
+ *     H = sum_j sum_a h^a_j S^a_j + sum_{j != k} sum_a J^a_{jk} S^a_j S^a_k ,   a = x, y, z,  S = Pauli / 2,
+ * the state |psi> = sum_k c_k |k> (eq. 2; 2^N complex doubles) is advanced by the 2nd- or 4th-order
+ * Trotter-Suzuki product formulas of P:54-58 in the paper's XYZ decomposition (eq. 6-10): diagonal
+ * phase sweeps exp(-i t E_a(k)) and per-spin pair rotations X, Y of eq. 5.
+ *
+ * Conventions (identical in the oracle):
+ *   - spin j (0-based) <-> bit j of the amplitude index k; bit = 1 is "up" (S^z = +1/2), 0 is "down".
+ *   - amplitudes are interleaved (re, im) IEEE doubles; amplitude k is at byte offset 16 k.
+ *   - alpha: TS_X = 0, TS_Y = 1, TS_Z = 2.  h is [3][N] row-major, J is [3][N][N] row-major.
+ *   - J need not be symmetric: the coupling of the unordered pair {j,k} is J[a][j][k] + J[a][k][j]; J[a][j][j] is
+ *     ignored (A1).
+ *   - U_1(t) = exp(-itH_x) exp(-itH_y) exp(-itH_z) (A6),  U_2(t) = U_1^dag(-t/2) U_1(t/2),
+ *     U_4(t) = U_2(at) U_2(at) U_2((1-4a)t) U_2(at) U_2(at),  a = 1/(4 - 4^(1/3)).
+ *   - no normalisation is ever applied; expectation values are <psi|S^a_j|psi>, not divided by <psi|psi>.
+ *
+ * Every call returns a status (TS_OK = 0 or a negative TS_ERR_*) and never throws or aborts.  Pointer arguments are
+ * HOST pointers unless the comment says "device".  A context is not thread-safe: use one per host thread.
+ * All work runs on the context's CUDA stream (default: the legacy default stream; see ts_set_stream).  Calls that
+ * return scalars to the host synchronise that stream; ts_evolve and the state setters do not (except host copies).
+ * There is no CPU fallback: every call that touches the state fails with TS_ERR_CUDA when no CUDA device is usable.
+ */
+#ifndef TS_B200_H
+#define TS_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ts_ctx ts_ctx; /* opaque; owns the device tables and (unless a buffer is bound) the state */
+
+enum { TS_OK = 0, TS_ERR_ARG = -1, TS_ERR_NOMEM = -2, TS_ERR_CUDA = -3, TS_ERR_NOSTATE = -4 };
+enum { TS_X = 0, TS_Y = 1, TS_Z = 2 };
+enum { TS_HOST = 0, TS_DEVICE = 1 };
+/* ts_set_plan modes */
+enum { TS_PLAN_AUTO = 0, TS_PLAN_NAIVE = 1, TS_PLAN_TILED = 2 };
+/* ts_get_profile kernel classes */
+enum { TS_KC_TILE_FUSED = 0,   /* tile pass: sweep . diagonal . sweep in one HBM round trip  */
+       TS_KC_TILE_SINGLE = 1,  /* tile pass: one sweep's butterflies on one bit group (+ optional diagonal) */
+       TS_KC_NAIVE_ROT = 2,    /* one-bit pair rotation, one launch per spin (the paper's basic kernel) */
+       TS_KC_NAIVE_DIAG = 3,   /* per-amplitude O(N^2) phase correction */
+       TS_KC_REDUCE = 4,       /* observable / norm reductions */
+       TS_KC_SETUP = 5,        /* phase-table construction, state initialisation */
+       TS_KC_COUNT = 6 };
+
+/* Problem statement (eq. 1).  N in [1, 33].  h: [3][N], J: [3][N][N]; both are COPIED.
+ * Errors: TS_ERR_ARG (null pointer, N out of range, non-finite h or J), TS_ERR_CUDA (no device), TS_ERR_NOMEM. */
+int ts_create(ts_ctx** out, int N, const double* h, const double* J);
+
+/* Frees the tables and the state if the library owns it.  NULL is accepted. */
+int ts_destroy(ts_ctx* ctx);
+
+/* Use this CUDA stream (a cudaStream_t passed as void*; NULL = legacy default stream) for all later work. */
+int ts_set_stream(ts_ctx* ctx, void* cuda_stream);
+
+/* Bind a caller-owned DEVICE buffer of 2^N complex128 (16 * 2^N bytes, 16-byte aligned) as the state vector
+ * (P:109).  The library evolves it IN PLACE and never frees it.  Any library-owned state is released. */
+int ts_bind_state(ts_ctx* ctx, void* dev_amps);
+
+/* Copy 2^N amplitudes into the state (eq. 2).  where = TS_HOST: amps is a host pointer (pinned or pageable;
+ * synchronous for pageable memory); TS_DEVICE: a device pointer (device-to-device copy).  If no buffer is bound the
+ * library allocates its own.  Errors: TS_ERR_ARG, TS_ERR_NOMEM. */
+int ts_set_state(ts_ctx* ctx, const void* amps, int where);
+
+/* State := basis state |k>  (c_k = 1, all others 0); allocates like ts_set_state.  k < 2^N. */
+int ts_set_basis_state(ts_ctx* ctx, uint64_t k);
+
+/* Copy amplitudes first .. first+count-1 to dst (host or device as `where`); synchronises for TS_HOST. */
+int ts_get_state(ts_ctx* ctx, void* dst, uint64_t first, uint64_t count, int where);
+
+/* psi <- [U_order(tau)]^n_steps psi  with order = 2 or 4; tau may be negative (echo, eq. 11);
+ * n_steps = 0 is a no-op.  Asynchronous on the stream.  One 4th-order step is 20 global rotations ("sweeps") and
+ * 20 merged diagonals; see DESIGN.md "Sequencer".  Errors: TS_ERR_ARG (order, n_steps < 0, non-finite tau),
+ * TS_ERR_NOSTATE, TS_ERR_CUDA. */
+int ts_evolve(ts_ctx* ctx, double tau, int64_t n_steps, int order);
+
+/* out[0] = <psi|S^alpha_j|psi>, j 0-based (reading A15).  Synchronises. */
+int ts_expect(ts_ctx* ctx, int alpha, int j, double* out);
+
+/* out[j] = <psi|S^alpha_j|psi> for all j < N (host array of N doubles).  Synchronises. */
+int ts_expect_all(ts_ctx* ctx, int alpha, double* out);
+
+/* out[0] = <psi|psi>.  Synchronises. */
+int ts_norm2(ts_ctx* ctx, double* out);
+
+/* out[0], out[1] = Re, Im of <phi|psi> where phi is a DEVICE buffer of 2^N complex128 (eq. 11). */
+int ts_overlap(ts_ctx* ctx, const void* dev_phi, double* out);
+
+/* Execution plan.  mode: TS_PLAN_AUTO (tiled when N >= 12, else naive), TS_PLAN_NAIVE (one launch per spin rotation
+ * and per diagonal: the paper's basic scheme, kept as bring-up path and A/B baseline), TS_PLAN_TILED.
+ * run_bits: number s of lowest index bits kept inside every high-bit tile (runs of 2^s * 16 bytes),
+ * 0 = default (3).  max_group_bits: upper bound on butterflied bits per high-bit pass, 0 = as many as fit
+ * (12 - s); smaller values force more passes (used by tests to exercise multi-group plans at small N).
+ * Errors: TS_ERR_ARG when the combination cannot be planned for this N. */
+int ts_set_plan(ts_ctx* ctx, int mode, int run_bits, int max_group_bits);
+
+/* Human-readable description of the current plan (groups, passes per sweep) into buf (NUL-terminated). */
+int ts_describe_plan(ts_ctx* ctx, char* buf, int buflen);
+
+/* Per-kernel-class device timing.  enable != 0: every later launch is bracketed by CUDA events on the stream.
+ * ts_get_profile synchronises, then writes, for class c in [0, TS_KC_COUNT): launches[c], ms[c] (sum of event
+ * durations) since the last ts_reset_profile.  Launch counts are kept even when timing is disabled (ms = 0). */
+int ts_set_profiling(ts_ctx* ctx, int enable);
+int ts_get_profile(ts_ctx* ctx, int64_t* launches /*[TS_KC_COUNT]*/, double* ms /*[TS_KC_COUNT]*/);
+int ts_reset_profile(ts_ctx* ctx);
+
+/* Static string for a status code. */
+const char* ts_strerror(int status);
+
+/* Library build info: "ts_b200 <version> sm_100a ..." */
+const char* ts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TS_B200_H */
