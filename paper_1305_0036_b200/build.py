@@ -15,7 +15,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libts_b200.so")
-SOURCES = ["ts_api.cu", "ts_tile.cu", "ts_naive.cu", "ts_reduce.cu"]
+SOURCES = ["ts_tile_cfgA.cu", "ts_tile_cfgH9.cu", "ts_tile_cfgG.cu", "ts_tile_cfgH10.cu", "ts_tile_cfgH8.cu",
+           "ts_tile_cfgH7.cu", "ts_api.cu", "ts_tile.cu", "ts_naive.cu", "ts_reduce.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -50,7 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             print(r.stderr)
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
     cmd = [nvcc, "-shared", "-o", LIB] + objs + ["-cudart", "static"]
     r = subprocess.run(cmd, capture_output=True, text=True)

@@ -106,8 +106,6 @@ int ensure_state(ts_ctx* c)
     return TS_OK;
 }
 
-struct DescKey { int alpha, scale_pow, group; double t; };
-
 } // namespace
 
 void ts_prof_begin(ts_ctx* c, int kc)
@@ -169,7 +167,6 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     }
     c->psi = nullptr; c->owns_psi = 0;
     c->plan_mode = TS_PLAN_AUTO; c->run_bits = 0; c->max_group_bits = 0;
-    c->d_desc = nullptr; c->desc_cap = 0;
     c->d_red = nullptr; c->red_cap = 0;
     c->profiling = 0;
     memset(c->launches, 0, sizeof(c->launches));
@@ -192,7 +189,7 @@ int ts_destroy(ts_ctx* c)
     if (c->psi && c->owns_psi) cudaFree(c->psi);
     if (c->d_h) cudaFree(c->d_h);
     if (c->d_Jeff) cudaFree(c->d_Jeff);
-    if (c->d_desc) cudaFree(c->d_desc);
+    ts_tile_free_tables(c);
     if (c->d_red) cudaFree(c->d_red);
     for (auto& r : c->recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto& e : c->ev_pool) cudaEventDestroy(e);
@@ -252,6 +249,8 @@ int ts_set_plan(ts_ctx* c, int mode, int run_bits, int max_group_bits)
     if (!c || mode < TS_PLAN_AUTO || mode > TS_PLAN_TILED || run_bits < 0 || max_group_bits < 0) return TS_ERR_ARG;
     const int om = c->plan_mode, orb = c->run_bits, omg = c->max_group_bits;
     c->plan_mode = mode; c->run_bits = run_bits; c->max_group_bits = max_group_bits;
+    cudaStreamSynchronize(c->stream);
+    ts_tile_free_tables(c);          // tables depend on the group geometry
     int st = build_plan(c);
     if (st != TS_OK) { c->plan_mode = om; c->run_bits = orb; c->max_group_bits = omg; build_plan(c); }
     return st;
@@ -297,36 +296,13 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
         return cuda_status(e);
     }
 
-    // phase-table descriptors, built on first use within this call (the step pattern repeats, so they are reused)
-    std::vector<DescKey> keys;
-    auto get_desc = [&](const DiagOp& d, int gi, const DiagDesc** out) -> cudaError_t {
-        for (size_t i = 0; i < keys.size(); ++i)
-            if (keys[i].alpha == d.alpha && keys[i].scale_pow == d.scale_pow && keys[i].group == gi && keys[i].t == d.t) {
-                *out = c->d_desc + i;
-                return cudaSuccess;
-            }
-        if ((int)keys.size() >= c->desc_cap) {
-            // grow; descriptors already referenced by queued launches must stay alive -> allocate generously once
-            if (c->desc_cap != 0) return cudaErrorMemoryAllocation;
-            cudaError_t ee = cudaMalloc(&c->d_desc, sizeof(DiagDesc) * 64);
-            if (ee != cudaSuccess) return ee;
-            c->desc_cap = 64;
-        }
-        DescKey k; k.alpha = d.alpha; k.scale_pow = d.scale_pow; k.group = gi; k.t = d.t;
-        keys.push_back(k);
-        DiagDesc* dst = c->d_desc + (keys.size() - 1);
-        *out = dst;
-        return ts_tile_build_desc(c, dst, d, c->groups[gi]);
-    };
     auto pass = [&](int gi, int k1, const DiagOp* d, int k2) -> cudaError_t {
-        const DiagDesc* dd = nullptr;
-        int alpha = 0;
+        const DiagTables* tb = nullptr;
         if (d && d->present) {
-            cudaError_t ee = get_desc(*d, gi, &dd);
+            cudaError_t ee = ts_tile_get_tables(c, *d, gi, &tb);
             if (ee != cudaSuccess) return ee;
-            alpha = d->alpha;
         }
-        return ts_tile_pass(c, c->groups[gi], k1, dd, k2, alpha);
+        return ts_tile_pass(c, gi, k1, tb, k2);
     };
 
     const int g = (int)c->groups.size();

@@ -38,20 +38,13 @@ struct TileGroup {
     int is_low;   // group A: butterflies all 12 tile bits; otherwise the 12 - s group bits
 };
 
-// Device-resident description of one (diagonal kind, tile group): tile-independent phase tables plus the spin lists
-// the per-tile preparation needs.  Built by ts_tile_build_desc (setup kernel, accurate sincos).
-struct DiagDesc {
-    double t;            // time of the diagonal
-    double scale;        // exact power of two
-    int alpha;
-    int N;
-    int nfixed;          // number of spins outside the tile
-    int rspin[5];        // spins held in the 5 register bits at diagonal time
-    int tspin[7];        // spins addressed by the 7 thread-index bits at diagonal time
-    int xspin[TS_MAX_FIXED]; // spins outside the tile, in tile-index bit order
-    double2 TT[128];     // exp(-it [E_T(t) - 1/2 sum_i b_i(t)])
-    double2 WT[5][128];  // exp(-it b_i(t)),  b_i(t) = sum_{j in T} Jeff_ij sigma_j(t)
-    double2 RR[32];      // exp(-it E_R(r))
+// Phase tables of one (diagonal kind, tile group), see ts_tile_kernel.cuh.  Built on first use, cached in the context.
+struct DiagTables {
+    int alpha, scale_pow, group;
+    double t;
+    double2* d_thread;       // device: TT[128] followed by WT[5][128]
+    double2* d_tile_phase;   // device: [ntiles][32]
+    double2 RR[32];          // host (passed to the kernel in its parameters)
 };
 
 struct ProfileRec { int kc; cudaEvent_t e0, e1; };
@@ -69,9 +62,8 @@ struct ts_ctx {
     // plan
     int plan_mode, run_bits, max_group_bits;
     std::vector<TileGroup> groups;
-    // diag descriptors (device), grown on demand
-    DiagDesc* d_desc;
-    int desc_cap;
+    // phase tables, built on demand and cached (invalidated when the plan changes)
+    std::vector<DiagTables> tabs;
     // reduction scratch
     double* d_red;
     size_t red_cap;   // in doubles
@@ -92,10 +84,10 @@ cudaError_t ts_naive_rotate(ts_ctx* c, int j, int kind);
 cudaError_t ts_naive_diag(ts_ctx* c, const DiagOp& d);
 
 // ---- tiled path (ts_tile.cu)
-cudaError_t ts_tile_build_desc(ts_ctx* c, DiagDesc* d_dst, const DiagOp& d, const TileGroup& g);
-cudaError_t ts_tile_pass(ts_ctx* c, const TileGroup& g, int kind1, const DiagDesc* d_desc /*or NULL*/, int kind2,
-                         int alpha /*of d_desc*/);
-cudaError_t ts_tile_init(void);   // sets max dynamic shared memory on all instantiations
+cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, const DiagTables** out);
+void ts_tile_free_tables(ts_ctx* c);
+cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tabs /*or NULL*/, int kind2);
+cudaError_t ts_tile_init(void);   // registers the kernels, sets max dynamic shared memory on all of them
 
 // ---- reductions (ts_reduce.cu)
 cudaError_t ts_reduce_expect_z_all(ts_ctx* c, double* out_host /*[N]*/);
