@@ -12,6 +12,7 @@
 // step in steady state.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -167,6 +168,8 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     }
     c->psi = nullptr; c->owns_psi = 0;
     c->plan_mode = TS_PLAN_AUTO; c->run_bits = 0; c->max_group_bits = 0;
+    c->chunk_log2 = getenv("TS_CHUNK_LOG2") ? atoi(getenv("TS_CHUNK_LOG2")) : 0;
+    c->chunks_per_launch = getenv("TS_CHUNKS_PER_LAUNCH") ? atoi(getenv("TS_CHUNKS_PER_LAUNCH")) : 1;
     c->d_red = nullptr; c->red_cap = 0;
     c->profiling = 0;
     memset(c->launches, 0, sizeof(c->launches));
@@ -296,40 +299,73 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
         return cuda_status(e);
     }
 
-    auto pass = [&](int gi, int k1, const DiagOp* d, int k2) -> cudaError_t {
-        const DiagTables* tb = nullptr;
-        if (d && d->present) {
-            cudaError_t ee = ts_tile_get_tables(c, *d, gi, &tb);
-            if (ee != cudaSuccess) return ee;
-        }
-        return ts_tile_pass(c, gi, k1, tb, k2);
+    // ---- pass list: one entry per HBM round trip (or per L2 round trip inside a blocked run)
+    struct Pass { int gi, k1, k2; DiagOp d; };
+    std::vector<Pass> passes;
+    auto push = [&](int gi, int k1, const DiagOp* d, int k2) {
+        Pass ps; ps.gi = gi; ps.k1 = k1; ps.k2 = k2;
+        if (d) ps.d = *d; else ps.d.present = 0;
+        passes.push_back(ps);
     };
-
     const int g = (int)c->groups.size();
-    for (int64_t i = 1; i <= q.M && e == cudaSuccess; ++i) {
+    for (int64_t i = 1; i <= q.M; ++i) {
         const bool fwd = (i & 1);
         if (g == 1) {
             const DiagOp d0 = q.diag(i - 1);
-            e = pass(0, SW_NONE, &d0, q.kind(i));
-            if (e == cudaSuccess && i == q.M) { const DiagOp dm = q.diag(q.M); e = pass(0, SW_NONE, &dm, SW_NONE); }
+            push(0, SW_NONE, &d0, q.kind(i));
+            if (i == q.M) { const DiagOp dm = q.diag(q.M); push(0, SW_NONE, &dm, SW_NONE); }
             continue;
         }
-        for (int pos = 0; pos < g && e == cudaSuccess; ++pos) {
+        for (int pos = 0; pos < g; ++pos) {
             const int gi = fwd ? pos : g - 1 - pos;
             const bool first = (pos == 0), last = (pos == g - 1);
             if (first && i > 1) continue;                              // done by the previous fused pass
             if (last && i < q.M) {                                     // sweep i . D_i . sweep i+1 on the same group
                 const DiagOp d = q.diag(i);
-                e = pass(gi, q.kind(i), &d, q.kind(i + 1));
+                push(gi, q.kind(i), &d, q.kind(i + 1));
             } else if (first && i == 1) {
                 const DiagOp d = q.diag(0);
-                e = pass(gi, SW_NONE, &d, q.kind(1));
+                push(gi, SW_NONE, &d, q.kind(1));
             } else if (last && i == q.M) {
                 const DiagOp d = q.diag(q.M);
-                e = pass(gi, q.kind(i), &d, SW_NONE);
+                push(gi, q.kind(i), &d, SW_NONE);
             } else {
-                e = pass(gi, q.kind(i), nullptr, SW_NONE);
+                push(gi, q.kind(i), nullptr, SW_NONE);
             }
+        }
+    }
+
+    auto launch = [&](const Pass& ps, uint64_t tile_base, uint64_t tile_count) -> cudaError_t {
+        const DiagTables* tb = nullptr;
+        if (ps.d.present) {
+            cudaError_t ee = ts_tile_get_tables(c, ps.d, ps.gi, &tb);
+            if (ee != cudaSuccess) return ee;
+        }
+        return ts_tile_pass(c, ps.gi, ps.k1, tb, ps.k2, tile_base, tile_count);
+    };
+
+    // ---- execution.  L2 blocking: consecutive passes whose groups all lie below spin
+    // `chunk_log2` act inside aligned chunks of 2^chunk_log2 amplitudes (closed-set argument of P:141 applied to the
+    // chunk), so such a run is executed chunk window by chunk window: the window is read from HBM by the first pass,
+    // stays in the 126 MB L2 for the passes in between and is written back once.
+    const int C = c->chunk_log2;
+    const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
+    auto top_spin = [&](int gi) { const TileGroup& t = c->groups[gi]; return t.is_low ? TS_TILE_LOG2 - 1 : t.g0 + TS_TILE_LOG2 - t.s - 1; };
+    size_t ip = 0;
+    while (ip < passes.size() && e == cudaSuccess) {
+        size_t jp = ip;
+        if (C > 0 && C < c->N)
+            while (jp < passes.size() && top_spin(passes[jp].gi) < C) ++jp;
+        if (jp - ip >= 2) {
+            const uint64_t win = ((uint64_t)1 << (C - TS_TILE_LOG2)) * (uint64_t)(c->chunks_per_launch > 0 ? c->chunks_per_launch : 1);
+            for (uint64_t tb0 = 0; tb0 < ntiles && e == cudaSuccess; tb0 += win) {
+                const uint64_t cnt = (ntiles - tb0 < win) ? ntiles - tb0 : win;
+                for (size_t k = ip; k < jp && e == cudaSuccess; ++k) e = launch(passes[k], tb0, cnt);
+            }
+            ip = jp;
+        } else {
+            e = launch(passes[ip], 0, 0);
+            ++ip;
         }
     }
     return cuda_status(e);

@@ -61,6 +61,7 @@ struct ts_ctx {
     int owns_psi;
     // plan
     int plan_mode, run_bits, max_group_bits;
+    int chunk_log2, chunks_per_launch;   // L2 blocking (0 = off)
     std::vector<TileGroup> groups;
     // phase tables, built on demand and cached (invalidated when the plan changes)
     std::vector<DiagTables> tabs;
@@ -86,7 +87,9 @@ cudaError_t ts_naive_diag(ts_ctx* c, const DiagOp& d);
 // ---- tiled path (ts_tile.cu)
 cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, const DiagTables** out);
 void ts_tile_free_tables(ts_ctx* c);
-cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tabs /*or NULL*/, int kind2);
+// tile_count = 0: all tiles; otherwise the window [tile_base, tile_base + tile_count)
+cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tabs /*or NULL*/, int kind2,
+                         uint64_t tile_base, uint64_t tile_count);
 cudaError_t ts_tile_init(void);   // registers the kernels, sets max dynamic shared memory on all of them
 
 // ---- reductions (ts_reduce.cu)

@@ -233,11 +233,13 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, const Diag
     return e;
 }
 
-cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tb, int kind2)
+cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tb, int kind2, uint64_t tile_base,
+                         uint64_t tile_count)
 {
     const TileGroup& g = c->groups[group];
     TilePassParams p;
     p.psi = c->psi;
+    p.tile_base = tile_base;
     p.tile_phase = nullptr; p.TT = nullptr; p.WT = nullptr; p.scale = 1.0;
     if (tb) {
         p.tile_phase = tb->d_tile_phase;
@@ -255,7 +257,7 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tb, 
     if (g.is_low) { p.bf1 = 31u; p.bf2 = 31u; }
     else if (nb <= 5) { p.bf1 = (31u << (5 - nb)) & 31u; p.bf2 = 0u; }          // top nb bits of f 7..11
     else { p.bf1 = 31u; p.bf2 = (31u << (10 - nb)) & 31u; }                       // top nb-5 bits of f 2..6
-    const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
+    const uint64_t ntiles = tile_count ? tile_count : (uint64_t)1 << (c->N - TS_TILE_LOG2);
     const size_t smem = p.two_stage ? (sizeof(double2) << TS_TILE_LOG2) : 0;
     tile_kernel_t k = g_tab[cfg_of(g)][kind1][kind2];
     if (!k) k = g_tab[TS_CFG_GENERIC][kind1][kind2];

@@ -47,6 +47,7 @@
 
 struct TilePassParams {
     double2* psi;
+    uint64_t tile_base;          // first tile of this launch (L2-blocked runs launch a window of tiles)
     const double2* tile_phase;   // [ntiles][32]   (NULL: no diagonal in this pass)
     const double2* TT;           // [128]
     const double2* WT;           // [5][128]
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __gri
 
     const int t = threadIdx.x;
     const int lane = t & 31;
-    const uint64_t tau = blockIdx.x;
+    const uint64_t tau = p.tile_base + blockIdx.x;
     const int s = p.s, g0 = p.g0;
     const int nmid = g0 - s;
     const uint64_t base_idx =
