@@ -23,6 +23,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_1305_0036_b200 import replicas as R  # noqa: E402
 from paper_1305_0036_b200 import workloads as W  # noqa: E402
 
 METRIC = "trotter_steps_per_sec"
@@ -170,7 +171,7 @@ def run_ours(args):
     N = args.N
     w = workload_for(N)
     if world > 1:                      # independent ensemble members: same Hamiltonian, different random state
-        w.state_seed = (w.state_seed or 0) + 1000 * rank
+        w.state_seed = R.replica_state_seed(w.state_seed, rank)
     dim = 1 << N
     ts = B.TrotterSuzuki(N, w.h, w.J, device=str(dev))
     if args.plan:
@@ -207,11 +208,8 @@ def run_ours(args):
     prof = ts.get_profile()
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     norm2 = ts.norm2()
-    if world > 1:
-        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-    steps_per_s = world * args.steps / (ms * 1e-3)
+    ms = R.max_over_ranks(ms, dev)
+    steps_per_s = R.whole_job_steps_per_s(args.steps, world, ms)
 
     # ---- end to end through the C ABI with host buffers: H2D of the state + 1 step + D2H of <S^z_j>
     e2e = None
@@ -226,11 +224,8 @@ def run_ours(args):
             sz = ts.expect_all(B.Z)                  # device -> host, N doubles (synchronises)
         barrier()
         te = time.perf_counter() - te
-        if world > 1:
-            tt = torch.tensor([te], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            te = float(tt.item())
-        e2e = {"value": world * n_e2e / te, "unit": UNIT, "h2d_bytes_per_step": 16 * dim,
+        te = R.max_over_ranks(te, dev)
+        e2e = {"value": R.whole_job_steps_per_s(n_e2e, world, te * 1e3), "unit": UNIT, "h2d_bytes_per_step": 16 * dim,
                "d2h_bytes_per_step": 8 * N, "steps": n_e2e,
                "what": "ts_set_state(pinned host) + ts_evolve(1 step) + ts_expect_all(z) per step"}
 

@@ -69,6 +69,11 @@ int ts_bind_state(ts_ctx* ctx, void* dev_amps);
  * library allocates its own.  Errors: TS_ERR_ARG, TS_ERR_NOMEM. */
 int ts_set_state(ts_ctx* ctx, const void* amps, int where);
 
+/* Copy `count` amplitudes to positions first .. first+count-1 of the state (chunked upload: an N = 32 state is 64 GiB,
+ * larger than most host buffers).  Allocates like ts_set_state; amplitudes outside the range are left as they are.
+ * Errors: TS_ERR_ARG (range outside [0, 2^N)), TS_ERR_NOMEM. */
+int ts_set_state_range(ts_ctx* ctx, const void* amps, uint64_t first, uint64_t count, int where);
+
 /* State := basis state |k>  (c_k = 1, all others 0); allocates like ts_set_state.  k < 2^N. */
 int ts_set_basis_state(ts_ctx* ctx, uint64_t k);
 

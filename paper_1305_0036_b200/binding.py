@@ -23,7 +23,7 @@ KC_COUNT = len(KC_NAMES)
 
 # every symbol include/ts_b200.h declares (tests check that the library exports all of them)
 SYMBOLS = ("ts_create", "ts_destroy", "ts_set_stream", "ts_bind_state", "ts_set_state", "ts_set_basis_state",
-           "ts_get_state", "ts_evolve", "ts_expect", "ts_expect_all", "ts_norm2", "ts_overlap", "ts_set_plan",
+           "ts_set_state_range", "ts_get_state", "ts_evolve", "ts_expect", "ts_expect_all", "ts_norm2", "ts_overlap", "ts_set_plan",
            "ts_describe_plan", "ts_set_profiling", "ts_get_profile", "ts_reset_profile", "ts_strerror", "ts_version")
 
 _lib = None
@@ -52,6 +52,7 @@ def load() -> ctypes.CDLL:
         "ts_set_stream": (I, [_vp, _vp]),
         "ts_bind_state": (I, [_vp, _vp]),
         "ts_set_state": (I, [_vp, _vp, I]),
+        "ts_set_state_range": (I, [_vp, _vp, U64, U64, I]),
         "ts_set_basis_state": (I, [_vp, U64]),
         "ts_get_state": (I, [_vp, _vp, U64, U64, I]),
         "ts_evolve": (I, [_vp, D, I64, I]),
@@ -152,6 +153,24 @@ class TrotterSuzuki:
                 raise ValueError("state must be a contiguous complex128 tensor with 2^N elements")
             where = DEVICE if amps.is_cuda else HOST
             _check(self._lib.ts_set_state(self._ctx, _vp(amps.data_ptr()), where), "ts_set_state")
+
+    def set_state_range(self, amps, first: int):
+        """Chunked upload: amps (numpy complex128, or a torch complex128 tensor on host/device) -> state[first:]."""
+        if isinstance(amps, np.ndarray):
+            a = np.ascontiguousarray(amps, dtype=np.complex128)
+            _check(self._lib.ts_set_state_range(self._ctx, _vp(a.ctypes.data), int(first), a.size, HOST),
+                   "ts_set_state_range")
+            self._stream.synchronize()      # `a` may be a temporary
+        else:
+            if amps.dtype != self._torch.complex128 or not amps.is_contiguous():
+                raise ValueError("chunk must be a contiguous complex128 tensor")
+            _check(self._lib.ts_set_state_range(self._ctx, _vp(amps.data_ptr()), int(first), amps.numel(),
+                                                DEVICE if amps.is_cuda else HOST), "ts_set_state_range")
+
+    def set_state_chunks(self, chunks):
+        """chunks: iterable of (first_index, numpy complex128 chunk), e.g. Workload.state_chunks()."""
+        for first, chunk in chunks:
+            self.set_state_range(chunk, first)
 
     def set_basis_state(self, k: int):
         _check(self._lib.ts_set_basis_state(self._ctx, int(k)), "ts_set_basis_state")

@@ -226,6 +226,19 @@ int ts_set_state(ts_ctx* c, const void* amps, int where)
     return cuda_status(e);
 }
 
+int ts_set_state_range(ts_ctx* c, const void* amps, uint64_t first, uint64_t count, int where)
+{
+    if (!c || !amps || (where != TS_HOST && where != TS_DEVICE)) return TS_ERR_ARG;
+    const uint64_t dim = (uint64_t)1 << c->N;
+    if (first > dim || count > dim - first) return TS_ERR_ARG;
+    int st = ensure_state(c);
+    if (st != TS_OK) return st;
+    if (count == 0) return TS_OK;
+    cudaError_t e = cudaMemcpyAsync(c->psi + first, amps, count * sizeof(double2),
+                                    where == TS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream);
+    return cuda_status(e);
+}
+
 int ts_set_basis_state(ts_ctx* c, uint64_t k)
 {
     if (!c || k >= ((uint64_t)1 << c->N)) return TS_ERR_ARG;

@@ -1,0 +1,180 @@
+"""GPU parity at the sizes no full CPU run can reach in test time.
+
+Cluster factorisation (SURVEY 8 c): if J couples spins only inside disjoint clusters and psi_0 is a product over the
+clusters, every factor of the product formulas -- each diagonal D_alpha(t) and each one-spin rotation -- is a tensor
+product over clusters, hence so are U_2 and U_4: any amplitude of the N = 27 / 30 / 32 state equals the product of the
+cluster amplitudes, which the ORACLE computes at N <= 11.  (That the oracle itself factorises this way is pinned on
+the CPU by tests/test_oracle_pins.py::test_cluster_factorisation_of_the_product_formulas.)  Clusters are interleaved
+bit sets (bit c, c + n_c, c + 2 n_c, ...), so their couplings cross every tile and group boundary of the CUDA path.
+Compared: >= 2^20 sampled amplitudes in windows at random unaligned offsets, and all <S^alpha_j>.
+
+Also: BASELINE config 4 (N = 27) against the full oracle, and the config-5 Hamiltonian (N = 32, 64 GiB in place) via
+properties that hold at any size (norm, echo) -- a full N = 32 oracle run takes hours on the box's 16 cores.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import ts_oracle as O
+from paper_1305_0036_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+AMP_TOL = 1e-11
+OBS_TOL = 1e-10
+FULL = os.environ.get("TS_PARITY_FULL", "0") == "1"
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1305_0036_b200 import binding
+    binding.load()
+    return binding
+
+
+def upload_cluster_product(ts, w, chunk_log2=24):
+    """psi_0[k] = prod_c state_c[bits_c(k)], built chunk by chunk ON the device (index gathers only: input
+    generation, none of the method's arithmetic) and handed to the library through ts_set_state_range."""
+    import torch
+    dev = ts.device
+    sts = [torch.from_numpy(s).to(dev) for s in w.cluster_states]
+    csz = 1 << min(chunk_log2, w.N)
+    for first in range(0, 1 << w.N, csz):
+        k = torch.arange(first, first + csz, dtype=torch.int64, device=dev)
+        c = None
+        for bits, st in zip(w.clusters, sts):
+            idx = torch.zeros_like(k)
+            for i, b in enumerate(bits):
+                idx |= ((k >> b) & 1) << i
+            c = st[idx] if c is None else c * st[idx]
+        ts.set_state_range(c.contiguous(), first)
+    torch.cuda.synchronize()
+
+
+def oracle_cluster_states(w, n_steps):
+    out = []
+    for ci in range(len(w.clusters)):
+        sub = W.sub_workload(w, ci)
+        psi = sub.state()
+        O.evolve(psi, sub.N, sub.h, sub.J, w.tau, n_steps, w.order, True)
+        out.append(psi)
+    return out
+
+
+def expected_amplitudes(w, subs, k):
+    c = np.ones(k.size, dtype=np.complex128)
+    for bits, st in zip(w.clusters, subs):
+        c *= st[W.extract_bits(k, bits)]
+    return c
+
+
+def expected_observables(w, subs):
+    """<S^alpha_j> of the product state = <S^alpha_j>_cluster * prod of the other clusters' norms."""
+    norms = [O.norm2(s, len(b)) for s, b in zip(subs, w.clusters)]
+    exp = np.zeros((3, w.N))
+    for ci, (bits, st) in enumerate(zip(w.clusters, subs)):
+        others = np.prod([n for i, n in enumerate(norms) if i != ci])
+        for a in range(3):
+            v = O.expect_all(st, len(bits), a)
+            for i, b in enumerate(bits):
+                exp[a, b] = v[i] * others
+    return exp, float(np.prod(norms))
+
+
+def check_clustered(B, N, n_clusters, n_steps, seed, n_windows=64, window=1 << 14, xy_sites=(0, 13)):
+    w = W.clustered(N, W.interleaved_clusters(N, n_clusters), seed=seed, tau=0.02, n_steps=n_steps)
+    ts = B.TrotterSuzuki(N, w.h, w.J)
+    upload_cluster_product(ts, w)
+    ts.evolve(w.tau, n_steps, 4)
+    subs = oracle_cluster_states(w, n_steps)
+    rng = np.random.Generator(np.random.PCG64(seed + 1))
+    dim = 1 << N
+    firsts = [0, dim - window] + [int(x) for x in rng.integers(0, dim - window, n_windows - 2)]
+    worst = 0.0
+    for first in firsts:
+        got = ts.get_state(first, window)
+        ref = expected_amplitudes(w, subs, np.arange(first, first + window, dtype=np.int64))
+        worst = max(worst, float(np.max(np.abs(got - ref))))
+    assert worst <= AMP_TOL, f"N={N}: max-abs {worst:.3e} over {n_windows * window} sampled amplitudes"
+    exp, n2 = expected_observables(w, subs)
+    assert np.max(np.abs(ts.expect_all(B.Z) - exp[2])) <= OBS_TOL
+    assert abs(ts.norm2() - n2) <= OBS_TOL
+    for j in xy_sites:                       # one pass per site: a couple of sites per axis
+        if j < N:
+            assert abs(ts.expect(B.X, j) - exp[0, j]) <= OBS_TOL
+            assert abs(ts.expect(B.Y, N - 1 - j) - exp[1, N - 1 - j]) <= OBS_TOL
+    plan = ts.describe_plan()
+    ts.close()
+    return plan
+
+
+def test_cluster_factorisation_N24_two_steps(B):
+    check_clustered(B, 24, 3, 2, seed=24)
+
+
+def test_cluster_factorisation_N27(B):
+    check_clustered(B, 27, 3, 2, seed=27)
+
+
+def test_cluster_factorisation_N30_bench_plan(B):
+    """The metric size in the launch configuration bench.py times (default plan)."""
+    plan = check_clustered(B, 30, 3, 1, seed=30)
+    assert "A[spins 0..11]" in plan and "3 group" in plan
+
+
+def test_cluster_factorisation_N32_in_place(B):
+    """64 GiB state, in place (config 5's size)."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80 * 2 ** 30:
+        pytest.skip("needs 80 GiB of free device memory")
+    check_clustered(B, 32, 3, 1, seed=32, n_windows=32)
+
+
+def test_config4_grid27_vs_full_oracle(B):
+    """BASELINE config 4: 4x7 grid minus one site (A16), 2 GiB state.  Default: 1 step (the oracle needs ~45 s per
+    step on 16 cores); TS_PARITY_FULL=1 runs the configured 50."""
+    w = W.config(4)
+    n = w.n_steps if FULL else 1
+    ts = B.TrotterSuzuki(w.N, w.h, w.J)
+    psi = w.state()
+    ts.set_state(psi)
+    ts.evolve(w.tau, n, 4)
+    O.evolve(psi, w.N, w.h, w.J, w.tau, n, 4, True)
+    got = ts.get_state()
+    d = got - psi
+    assert np.max(np.abs(d)) <= AMP_TOL
+    assert np.linalg.norm(d) <= AMP_TOL
+    assert np.max(np.abs(ts.expect_all(B.Z) - O.expect_all(psi, w.N, 2))) <= OBS_TOL
+    ts.close()
+
+
+def test_config5_grid32_properties(B):
+    """BASELINE config 5 Hamiltonian and checkerboard Neel state at N = 32: properties that hold at any size.
+    Norm is conserved to 1e-12; the echo (U_4 is palindromic, so U_4(-tau) U_4(tau) = 1 exactly) returns the
+    Neel state: c_Neel = 1 and <S^z_j> = -+1/2 again.  (Oracle parity at this size: the cluster test above.)"""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80 * 2 ** 30:
+        pytest.skip("needs 80 GiB of free device memory")
+    w = W.config(5)
+    n = w.n_steps if FULL else 2
+    ts = B.TrotterSuzuki(w.N, w.h, w.J)
+    ts.set_basis_state(w.basis_index)
+    sz0 = ts.expect_all(B.Z)
+    assert np.all(np.abs(np.abs(sz0) - 0.5) == 0.0)
+    ts.evolve(w.tau, n, 4)
+    assert abs(ts.norm2() - 1.0) <= 1e-12
+    sz1 = ts.expect_all(B.Z)
+    assert 1e-6 < np.max(np.abs(sz1 - sz0)) < 0.1          # it moved, a little (tau * n = 0.02 .. 0.1)
+    assert abs(np.sum(sz1) - np.sum(sz0)) < 1e-2            # h^x is weak: total S^z nearly conserved
+    ts.evolve(-w.tau, n, 4)
+    c = ts.get_state(w.basis_index, 1)[0]
+    assert abs(c - 1.0) <= AMP_TOL
+    assert np.max(np.abs(ts.expect_all(B.Z) - sz0)) <= OBS_TOL
+    assert abs(ts.norm2() - 1.0) <= 1e-12
+    ts.close()
