@@ -48,7 +48,8 @@ enum { TS_KC_TILE_FUSED = 0,   /* tile pass: sweep . diagonal . sweep in one HBM
        TS_KC_NAIVE_DIAG = 3,   /* per-amplitude O(N^2) phase correction */
        TS_KC_REDUCE = 4,       /* observable / norm reductions */
        TS_KC_SETUP = 5,        /* phase-table construction, state initialisation */
-       TS_KC_COUNT = 6 };
+       TS_KC_TILE_CHUNK = 6,   /* three tile passes (high . fused low . high) in one L2-blocked launch: 1 HBM round trip */
+       TS_KC_COUNT = 7 };
 
 /* Problem statement (eq. 1).  N in [1, 33].  h: [3][N], J: [3][N][N]; both are COPIED.
  * Errors: TS_ERR_ARG (null pointer, N out of range, non-finite h or J), TS_ERR_CUDA (no device), TS_ERR_NOMEM. */

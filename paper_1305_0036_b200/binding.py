@@ -18,7 +18,7 @@ TS_OK, TS_ERR_ARG, TS_ERR_NOMEM, TS_ERR_CUDA, TS_ERR_NOSTATE = 0, -1, -2, -3, -4
 X, Y, Z = 0, 1, 2
 HOST, DEVICE = 0, 1
 PLAN_AUTO, PLAN_NAIVE, PLAN_TILED = 0, 1, 2
-KC_NAMES = ("tile_fused", "tile_single", "naive_rot", "naive_diag", "reduce", "setup")
+KC_NAMES = ("tile_fused", "tile_single", "naive_rot", "naive_diag", "reduce", "setup", "tile_chunk3")
 KC_COUNT = len(KC_NAMES)
 
 # every symbol include/ts_b200.h declares (tests check that the library exports all of them)

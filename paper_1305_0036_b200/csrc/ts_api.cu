@@ -170,6 +170,11 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->plan_mode = TS_PLAN_AUTO; c->run_bits = 0; c->max_group_bits = 0;
     c->chunk_log2 = getenv("TS_CHUNK_LOG2") ? atoi(getenv("TS_CHUNK_LOG2")) : 0;
     c->chunks_per_launch = getenv("TS_CHUNKS_PER_LAUNCH") ? atoi(getenv("TS_CHUNKS_PER_LAUNCH")) : 1;
+    c->pipe_mode = getenv("TS_PIPE") ? atoi(getenv("TS_PIPE")) : 1;
+    c->chunk_mode = getenv("TS_CHUNK3") ? atoi(getenv("TS_CHUNK3")) : 0;
+    c->chunk_max_log2 = getenv("TS_CHUNK3_MAX_LOG2") ? atoi(getenv("TS_CHUNK3_MAX_LOG2")) : 21;
+    c->d_sched = nullptr; c->d_chunk_ctr = nullptr; c->sched_nchunks = 0;
+    c->tmap_psi = nullptr;
     c->d_red = nullptr; c->red_cap = 0;
     c->profiling = 0;
     memset(c->launches, 0, sizeof(c->launches));
@@ -194,6 +199,8 @@ int ts_destroy(ts_ctx* c)
     if (c->d_Jeff) cudaFree(c->d_Jeff);
     ts_tile_free_tables(c);
     if (c->d_red) cudaFree(c->d_red);
+    if (c->d_sched) cudaFree(c->d_sched);
+    if (c->d_chunk_ctr) cudaFree(c->d_chunk_ctr);
     for (auto& r : c->recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto& e : c->ev_pool) cudaEventDestroy(e);
     delete c;
@@ -267,6 +274,7 @@ int ts_set_plan(ts_ctx* c, int mode, int run_bits, int max_group_bits)
     c->plan_mode = mode; c->run_bits = run_bits; c->max_group_bits = max_group_bits;
     cudaStreamSynchronize(c->stream);
     ts_tile_free_tables(c);          // tables depend on the group geometry
+    c->tmaps.clear();
     int st = build_plan(c);
     if (st != TS_OK) { c->plan_mode = om; c->run_bits = orb; c->max_group_bits = omg; build_plan(c); }
     return st;
@@ -366,6 +374,18 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
     auto top_spin = [&](int gi) { const TileGroup& t = c->groups[gi]; return t.is_low ? TS_TILE_LOG2 - 1 : t.g0 + TS_TILE_LOG2 - t.s - 1; };
     size_t ip = 0;
     while (ip < passes.size() && e == cudaSuccess) {
+        // [H single ka] [A fused ka . D . kb] [H single kb]  ->  one L2-blocked launch (ts_tile_chunk.cuh)
+        if (ip + 2 < passes.size()) {
+            const Pass &p0 = passes[ip], &p1 = passes[ip + 1], &p2 = passes[ip + 2];
+            if (p0.gi == p2.gi && p1.gi == 0 && p0.k2 == SW_NONE && !p0.d.present && p2.k2 == SW_NONE && !p2.d.present &&
+                p1.d.present && p1.k1 == p0.k1 && p1.k2 == p2.k1 && ts_tile_chunk_supported(c, p0.gi, p1.k1, p1.k2)) {
+                const DiagTables* tb = nullptr;
+                e = ts_tile_get_tables(c, p1.d, 0, &tb);
+                if (e == cudaSuccess) e = ts_tile_chunk_triple(c, p0.gi, p1.k1, tb, p1.k2);
+                ip += 3;
+                continue;
+            }
+        }
         size_t jp = ip;
         if (C > 0 && C < c->N)
             while (jp < passes.size() && top_spin(passes[jp].gi) < C) ++jp;

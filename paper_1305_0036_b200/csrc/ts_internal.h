@@ -47,6 +47,13 @@ struct DiagTables {
     double2 RR[32];          // host (passed to the kernel in its parameters)
 };
 
+// Cached CUtensorMap (128 bytes, kept opaque here so that this header does not need <cuda.h>).
+struct TensorMapSlot {
+    int valid;
+    alignas(64) unsigned char bytes[128];
+    TensorMapSlot() : valid(0) {}
+};
+
 struct ProfileRec { int kc; cudaEvent_t e0, e1; };
 
 struct ts_ctx {
@@ -62,6 +69,13 @@ struct ts_ctx {
     // plan
     int plan_mode, run_bits, max_group_bits;
     int chunk_log2, chunks_per_launch;   // L2 blocking (0 = off)
+    int chunk_mode, chunk_max_log2;      // L2-blocked triple launches (ts_tile_chunk.cuh): on/off, largest chunk (log2 amplitudes)
+    uint32_t* d_sched;                   // job-block order of the triple launch, for sched_nchunks chunks
+    unsigned int* d_chunk_ctr;           // ticket + done counters
+    uint32_t sched_nchunks;
+    int pipe_mode;                       // 1: persistent TMA-pipelined tile kernels (ts_tile_pipe.cuh), 0: one CTA per tile
+    std::vector<TensorMapSlot> tmaps;    // per group, for the bound state pointer tmap_psi
+    void* tmap_psi;
     std::vector<TileGroup> groups;
     // phase tables, built on demand and cached (invalidated when the plan changes)
     std::vector<DiagTables> tabs;
@@ -90,6 +104,9 @@ void ts_tile_free_tables(ts_ctx* c);
 // tile_count = 0: all tiles; otherwise the window [tile_base, tile_base + tile_count)
 cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tabs /*or NULL*/, int kind2,
                          uint64_t tile_base, uint64_t tile_count);
+bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb);
+// [H(gh) single ka] [A fused ka . D(tabs) . kb] [H(gh) single kb] in one L2-blocked launch
+cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagTables* tabs, int kb);
 cudaError_t ts_tile_init(void);   // registers the kernels, sets max dynamic shared memory on all of them
 
 // ---- reductions (ts_reduce.cu)

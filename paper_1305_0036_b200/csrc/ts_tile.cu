@@ -3,12 +3,21 @@
 #include <math.h>
 #include <string.h>
 
-#include "ts_tile_kernel.cuh"
+#include <cudaTypedefs.h>
+#include <stdio.h>
+#include <stdlib.h>
+
+#include "ts_tile_chunk.cuh"
+#include "ts_tile_pipe.cuh"
 
 namespace {
 
 tile_kernel_t g_tab[TS_CFG_COUNT][5][5];
+pipe_kernel_t g_pipe[TS_CFG_COUNT][5][5];
+chunk_kernel_t g_chunk[TS_CFG_COUNT][2];
 bool g_registered = false;
+int g_num_sms = 0;
+PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
 
 // Geometry of the diagonal-time layout of one group: which spins sit on register bits (R), thread bits (T) and
 // outside the tile (X).
@@ -171,8 +180,49 @@ cudaError_t ts_tile_init(void)
         ts_tile_register_H8(&g_tab[TS_CFG_H8]);
         ts_tile_register_H9(&g_tab[TS_CFG_H9]);
         ts_tile_register_H10(&g_tab[TS_CFG_H10]);
+        memset(g_pipe, 0, sizeof(g_pipe));
+        ts_pipe_register_generic(&g_pipe[TS_CFG_GENERIC]);
+        ts_pipe_register_A(&g_pipe[TS_CFG_A]);
+        ts_pipe_register_H7(&g_pipe[TS_CFG_H7]);
+        ts_pipe_register_H8(&g_pipe[TS_CFG_H8]);
+        ts_pipe_register_H9(&g_pipe[TS_CFG_H9]);
+        ts_pipe_register_H10(&g_pipe[TS_CFG_H10]);
+        memset(g_chunk, 0, sizeof(g_chunk));
+        ts_chunk_register_H7(&g_chunk[TS_CFG_H7]);
+        ts_chunk_register_H8(&g_chunk[TS_CFG_H8]);
+        ts_chunk_register_H9(&g_chunk[TS_CFG_H9]);
+        ts_chunk_register_H10(&g_chunk[TS_CFG_H10]);
         g_registered = true;
     }
+    if (!g_num_sms) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+    }
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+        if (e != cudaSuccess) return e;
+        if (qr != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+        g_encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
+    }
+    for (int cf = 0; cf < TS_CFG_COUNT; ++cf)
+        for (int v = 0; v < 2; ++v)
+            if (g_chunk[cf][v]) {
+                cudaError_t e = cudaFuncSetAttribute((const void*)g_chunk[cf][v], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                     (int)(sizeof(double2) << TS_TILE_LOG2));
+                if (e != cudaSuccess) return e;
+            }
+    for (int cf = 0; cf < TS_CFG_COUNT; ++cf)
+        for (int k1 = 0; k1 < 5; ++k1)
+            for (int k2 = 0; k2 < 5; ++k2)
+                if (g_pipe[cf][k1][k2]) {
+                    cudaError_t e = cudaFuncSetAttribute((const void*)g_pipe[cf][k1][k2],
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, TS_PIPE_SMEM);
+                    if (e != cudaSuccess) return e;
+                }
     for (int cf = 0; cf < TS_CFG_COUNT; ++cf)
         for (int k1 = 0; k1 < 5; ++k1)
             for (int k2 = 0; k2 < 5; ++k2)
@@ -233,6 +283,36 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, const Diag
     return e;
 }
 
+// Tensor map of a high group with short runs: the state seen as [hi][2^m rows][2^g0 amplitudes = 2^(g0+1) doubles];
+// one box = {2^s amplitudes, <= 256 rows, 1} (runs of 2^s consecutive elements, strided rows).
+cudaError_t ts_tile_tensor_map(ts_ctx* c, int group, CUtensorMap* out)
+{
+    if (c->tmap_psi != (void*)c->psi || c->tmaps.size() != c->groups.size()) {
+        c->tmaps.assign(c->groups.size(), TensorMapSlot());
+        c->tmap_psi = (void*)c->psi;
+    }
+    TensorMapSlot& sl = c->tmaps[group];
+    if (!sl.valid) {
+        const TileGroup& g = c->groups[group];
+        const int m = TS_TILE_LOG2 - g.s;
+        const int rows_half = 1 << (m - 1);
+        const int top = c->N - g.g0 - m;                     // index bits above the group
+        cuuint64_t dims[3] = {(cuuint64_t)2 << g.g0, (cuuint64_t)1 << m, (cuuint64_t)1 << top};
+        cuuint64_t strides[2] = {(cuuint64_t)16 << g.g0, (cuuint64_t)16 << (g.g0 + m)};
+        cuuint32_t box[3] = {(cuuint32_t)2 << g.s, (cuuint32_t)(rows_half < 256 ? rows_half : 256), 1};
+        cuuint32_t estr[3] = {1, 1, 1};
+        CUtensorMap tm;
+        CUresult r = g_encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)c->psi, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+        memcpy(sl.bytes, &tm, sizeof(tm));
+        sl.valid = 1;
+    }
+    memcpy(out, sl.bytes, sizeof(CUtensorMap));
+    return cudaSuccess;
+}
+
 cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tb, int kind2, uint64_t tile_base,
                          uint64_t tile_count)
 {
@@ -263,8 +343,134 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tb, 
     if (!k) k = g_tab[TS_CFG_GENERIC][kind1][kind2];
     if (!k) return cudaErrorInvalidValue;
     const bool fused = (kind1 != SW_NONE && kind2 != SW_NONE);
+    if (c->pipe_mode == 2 || (c->pipe_mode == 1 && fused)) {
+        pipe_kernel_t pk = g_pipe[cfg_of(g)][kind1][kind2];
+        if (!pk) pk = g_pipe[TS_CFG_GENERIC][kind1][kind2];
+        if (!pk) return cudaErrorInvalidValue;
+        PipeGeom pg;
+        pg.ntiles = ntiles;
+        pg.is_low = g.is_low;
+        const int m = TS_TILE_LOG2 - g.s;                  // rows per tile = 2^m (A: one row)
+        pg.row_bytes = g.is_low ? TS_PIPE_HALF_BYTES : (16 << g.s);
+        pg.rows_half = g.is_low ? 1 : (1 << (m - 1));
+        pg.tensor = (!g.is_low && g.s <= 7) ? 1 : 0;       // box inner dimension <= 256 doubles
+        pg.box_rows = pg.rows_half < 256 ? pg.rows_half : 256;
+        pg.nbox = pg.rows_half / pg.box_rows;
+        CUtensorMap tm;
+        memset(&tm, 0, sizeof(tm));
+        if (pg.tensor) {
+            cudaError_t e = ts_tile_tensor_map(c, group, &tm);
+            if (e != cudaSuccess) return e;
+        }
+        pg.dbg = nullptr;
+        if (getenv("TS_DEBUG")) { cudaMalloc(&pg.dbg, 64); cudaMemset(pg.dbg, 0, 64); }
+        const uint64_t grid = ntiles < (uint64_t)g_num_sms ? ntiles : (uint64_t)g_num_sms;
+        ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE);
+        pk<<<(unsigned)grid, TS_PIPE_THREADS, TS_PIPE_SMEM, c->stream>>>(p, tm, pg);
+        ts_prof_end(c);
+        if (getenv("TS_DEBUG")) {
+            cudaError_t e = cudaStreamSynchronize(c->stream);
+            fprintf(stderr, "pipe pass: group %d (s=%d g0=%d low=%d) k1=%d k2=%d diag=%d tensor=%d rows_half=%d row_bytes=%d "
+                    "box_rows=%d nbox=%d grid=%llu ntiles=%llu -> %s\n", group, g.s, g.g0, g.is_low, kind1, kind2, tb != nullptr,
+                    pg.tensor, pg.rows_half, pg.row_bytes, pg.box_rows, pg.nbox, (unsigned long long)grid,
+                    (unsigned long long)ntiles, cudaGetErrorString(e));
+            unsigned long long hd[5] = {0, 0, 0, 0, 0};
+            if (e == cudaSuccess) cudaMemcpy(hd, pg.dbg, sizeof(hd), cudaMemcpyDeviceToHost);
+            fprintf(stderr, "    landed-vs-global mismatches %llu (first: tile %llu reg %llu thread %llu slot %llu)\n", hd[0], hd[1],
+                    hd[2], hd[3], hd[4]);
+            cudaFree(pg.dbg);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaGetLastError();
+    }
     ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE);
     k<<<(unsigned)ntiles, TS_TILE_THREADS, smem, c->stream>>>(p);
+    ts_prof_end(c);
+    return cudaGetLastError();
+}
+
+namespace {
+
+void fill_params(const ts_ctx* c, const TileGroup& g, const DiagTables* tb, TilePassParams* p)
+{
+    p->psi = c->psi;
+    p->tile_base = 0;
+    p->tile_phase = nullptr; p->TT = nullptr; p->WT = nullptr; p->scale = 1.0;
+    if (tb) {
+        p->tile_phase = tb->d_tile_phase;
+        p->TT = tb->d_thread;
+        p->WT = tb->d_thread + 128;
+        p->scale = ldexp(1.0, tb->scale_pow);
+        memcpy(p->RR, tb->RR, sizeof(p->RR));
+    } else {
+        for (int r = 0; r < 32; ++r) p->RR[r] = make_double2(1.0, 0.0);
+    }
+    p->s = g.s; p->g0 = g.g0;
+    const int nb = n_bfly(g);
+    p->two_stage = two_stage(g) ? 1 : 0;
+    p->nshfl = g.is_low ? 2 : 0;
+    if (g.is_low) { p->bf1 = 31u; p->bf2 = 31u; }
+    else if (nb <= 5) { p->bf1 = (31u << (5 - nb)) & 31u; p->bf2 = 0u; }
+    else { p->bf1 = 31u; p->bf2 = (31u << (10 - nb)) & 31u; }
+}
+
+} // namespace
+
+// Can [H(gh) single ka] [A fused ka . D . kb] [H(gh) single kb] run as one L2-blocked launch?
+bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
+{
+    if (c->chunk_mode == 0 || gh < 1 || gh >= (int)c->groups.size() || !c->groups[0].is_low) return false;
+    const TileGroup& g = c->groups[gh];
+    if (g.g0 != TS_TILE_LOG2) return false;                            // the group right above A
+    const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
+    if (C >= c->N || C > c->chunk_max_log2) return false;
+    const int v = (ka == SW_YDAG && kb == SW_Y) ? 0 : (ka == SW_X && kb == SW_XDAG) ? 1 : -1;
+    return v >= 0 && g_chunk[cfg_of(g)][v] != nullptr;
+}
+
+cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagTables* tb, int kb)
+{
+    const TileGroup& g = c->groups[gh];
+    const int C = g.g0 + (TS_TILE_LOG2 - g.s);
+    const uint32_t nchunks = 1u << (c->N - C);
+    const uint32_t nblocks = 3 * nchunks;
+    if (c->sched_nchunks != nchunks) {
+        if (c->d_sched) cudaFree(c->d_sched);
+        if (c->d_chunk_ctr) cudaFree(c->d_chunk_ctr);
+        c->d_sched = nullptr; c->d_chunk_ctr = nullptr; c->sched_nchunks = 0;
+        std::vector<uint32_t> sched;
+        // P1(0) P2(0) | P1(k) P3(k-1) P2(k) ... | P3(last)
+        sched.push_back(0u | (0u << 2));
+        sched.push_back(1u | (0u << 2));
+        for (uint32_t k = 1; k < nchunks; ++k) {
+            sched.push_back(0u | (k << 2));
+            sched.push_back(2u | ((k - 1) << 2));
+            sched.push_back(1u | (k << 2));
+        }
+        sched.push_back(2u | ((nchunks - 1) << 2));
+        cudaError_t e = cudaMalloc(&c->d_sched, sizeof(uint32_t) * nblocks);
+        if (e == cudaSuccess) e = cudaMalloc(&c->d_chunk_ctr, sizeof(unsigned int) * (64 + 2 * (size_t)nchunks));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_sched, sched.data(), sizeof(uint32_t) * nblocks, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);    // `sched` is a temporary
+        if (e != cudaSuccess) return e;
+        c->sched_nchunks = nchunks;
+    }
+    ChunkParams q;
+    fill_params(c, g, nullptr, &q.h);
+    fill_params(c, c->groups[0], tb, &q.a);
+    q.sched = c->d_sched;
+    q.ticket = c->d_chunk_ctr;
+    q.done = c->d_chunk_ctr + 64;
+    q.nblocks = nblocks; q.nchunks = nchunks; q.tiles_log2 = (uint32_t)(C - TS_TILE_LOG2);
+    cudaError_t e = cudaMemsetAsync(c->d_chunk_ctr, 0, sizeof(unsigned int) * (64 + 2 * (size_t)nchunks), c->stream);
+    if (e != cudaSuccess) return e;
+    const int v = (ka == SW_YDAG) ? 0 : 1;
+    chunk_kernel_t k = g_chunk[cfg_of(g)][v];
+    const uint64_t jobs = (uint64_t)nblocks << q.tiles_log2;
+    uint64_t grid = 2 * (uint64_t)g_num_sms;
+    if (grid > jobs) grid = jobs;
+    ts_prof_begin(c, TS_KC_TILE_CHUNK);
+    k<<<(unsigned)grid, TS_TILE_THREADS, sizeof(double2) << TS_TILE_LOG2, c->stream>>>(q);
     ts_prof_end(c);
     return cudaGetLastError();
 }

@@ -181,17 +181,18 @@ __device__ __forceinline__ void apply_diag(const TilePassParams& p, double2 base
     }
 }
 
-template <int K1, int K2, int BF1, int BF2, int NSHFL, int MINB>
-__global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __grid_constant__ TilePassParams p)
+// One tile: load (layout 1), sweep K1, diagonal, sweep K2, store in place.  CG bit 0: bypass L1 on the loads
+// (ld.global.cg; needed when another SM wrote the tile earlier in the SAME launch, see ts_tile_chunk.cuh); bit 1: keep
+// the stores in L2 (st.global.cg) instead of streaming them out (st.global.cs).
+template <int K1, int K2, int BF1, int BF2, int NSHFL, int CG>
+__device__ __forceinline__ void tile_body(const TilePassParams& p, const uint64_t tau, double2* sm)
 {
-    extern __shared__ double2 sm[];          // 4096 slots when layout 2 is used
     constexpr bool GENERIC = (BF1 < 0);
     const bool two_stage = GENERIC ? (p.two_stage != 0) : (BF2 != 0);
     const int nshfl = GENERIC ? p.nshfl : NSHFL;
 
     const int t = threadIdx.x;
     const int lane = t & 31;
-    const uint64_t tau = p.tile_base + blockIdx.x;
     const int s = p.s, g0 = p.g0;
     const int nmid = g0 - s;
     const uint64_t base_idx =
@@ -214,7 +215,7 @@ __global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __gri
         uint64_t o = 0;
 #pragma unroll
         for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
-        const double2 v = __ldcs(gp + o);
+        const double2 v = (CG & 1) ? __ldcg(gp + o) : __ldcs(gp + o);
         re[r] = v.x; im[r] = v.y;
     }
 
@@ -253,8 +254,16 @@ __global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __gri
         uint64_t o = 0;
 #pragma unroll
         for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
-        __stcs(gp + o, make_double2(re[r], im[r]));
+        if (CG & 2) __stcg(gp + o, make_double2(re[r], im[r]));
+        else __stcs(gp + o, make_double2(re[r], im[r]));
     }
+}
+
+template <int K1, int K2, int BF1, int BF2, int NSHFL, int MINB>
+__global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __grid_constant__ TilePassParams p)
+{
+    extern __shared__ double2 sm[];          // 4096 slots when layout 2 is used
+    tile_body<K1, K2, BF1, BF2, NSHFL, 0>(p, p.tile_base + blockIdx.x, sm);
 }
 
 // The kernels a configuration needs: 4 fused transitions, 4 single sweeps, and "diagonal, then X^dag" (first pass).
