@@ -171,7 +171,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->chunk_log2 = getenv("TS_CHUNK_LOG2") ? atoi(getenv("TS_CHUNK_LOG2")) : 0;
     c->chunks_per_launch = getenv("TS_CHUNKS_PER_LAUNCH") ? atoi(getenv("TS_CHUNKS_PER_LAUNCH")) : 1;
     c->pipe_mode = getenv("TS_PIPE") ? atoi(getenv("TS_PIPE")) : 1;
-    c->chunk_mode = getenv("TS_CHUNK3") ? atoi(getenv("TS_CHUNK3")) : 0;
+    c->chunk_mode = getenv("TS_CHUNK3") ? atoi(getenv("TS_CHUNK3")) : 2;
     c->chunk_max_log2 = getenv("TS_CHUNK3_MAX_LOG2") ? atoi(getenv("TS_CHUNK3_MAX_LOG2")) : 21;
     c->d_sched = nullptr; c->d_chunk_ctr = nullptr; c->sched_nchunks = 0;
     c->tmap_psi = nullptr;

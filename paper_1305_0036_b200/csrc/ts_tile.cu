@@ -15,6 +15,7 @@ namespace {
 tile_kernel_t g_tab[TS_CFG_COUNT][5][5];
 pipe_kernel_t g_pipe[TS_CFG_COUNT][5][5];
 chunk_kernel_t g_chunk[TS_CFG_COUNT][2];
+chunk_pipe_kernel_t g_chunk_pipe[TS_CFG_COUNT][2];
 bool g_registered = false;
 int g_num_sms = 0;
 PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
@@ -192,6 +193,11 @@ cudaError_t ts_tile_init(void)
         ts_chunk_register_H8(&g_chunk[TS_CFG_H8]);
         ts_chunk_register_H9(&g_chunk[TS_CFG_H9]);
         ts_chunk_register_H10(&g_chunk[TS_CFG_H10]);
+        memset(g_chunk_pipe, 0, sizeof(g_chunk_pipe));
+        ts_chunk_pipe_register_H7(&g_chunk_pipe[TS_CFG_H7]);
+        ts_chunk_pipe_register_H8(&g_chunk_pipe[TS_CFG_H8]);
+        ts_chunk_pipe_register_H9(&g_chunk_pipe[TS_CFG_H9]);
+        ts_chunk_pipe_register_H10(&g_chunk_pipe[TS_CFG_H10]);
         g_registered = true;
     }
     if (!g_num_sms) {
@@ -213,6 +219,8 @@ cudaError_t ts_tile_init(void)
             if (g_chunk[cf][v]) {
                 cudaError_t e = cudaFuncSetAttribute((const void*)g_chunk[cf][v], cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                      (int)(sizeof(double2) << TS_TILE_LOG2));
+                if (e == cudaSuccess)
+                    e = cudaFuncSetAttribute((const void*)g_chunk_pipe[cf][v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_PIPE_SMEM);
                 if (e != cudaSuccess) return e;
             }
     for (int cf = 0; cf < TS_CFG_COUNT; ++cf)
@@ -283,6 +291,20 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, const Diag
     return e;
 }
 
+static void fill_pipe_geom(const TileGroup& g, uint64_t ntiles, PipeGeom* pg)
+{
+    pg->ntiles = ntiles;
+    pg->is_low = g.is_low;
+    const int m = TS_TILE_LOG2 - g.s;                  // rows per tile = 2^m (A: one row)
+    pg->row_bytes = g.is_low ? TS_PIPE_HALF_BYTES : (16 << g.s);
+    pg->rows_half = g.is_low ? 1 : (1 << (m - 1));
+    pg->tensor = (!g.is_low && g.s <= 7) ? 1 : 0;      // box inner dimension <= 256 doubles
+    pg->box_rows = pg->rows_half < 256 ? pg->rows_half : 256;
+    pg->nbox = pg->rows_half / pg->box_rows;
+    pg->dbg = nullptr;
+    pg->pf = getenv("TS_PF") ? atoi(getenv("TS_PF")) : 0;    // measured: L2 prefetches cost TMA issue time, slower at any distance
+}
+
 // Tensor map of a high group with short runs: the state seen as [hi][2^m rows][2^g0 amplitudes = 2^(g0+1) doubles];
 // one box = {2^s amplitudes, <= 256 rows, 1} (runs of 2^s consecutive elements, strided rows).
 cudaError_t ts_tile_tensor_map(ts_ctx* c, int group, CUtensorMap* out)
@@ -348,21 +370,13 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tb, 
         if (!pk) pk = g_pipe[TS_CFG_GENERIC][kind1][kind2];
         if (!pk) return cudaErrorInvalidValue;
         PipeGeom pg;
-        pg.ntiles = ntiles;
-        pg.is_low = g.is_low;
-        const int m = TS_TILE_LOG2 - g.s;                  // rows per tile = 2^m (A: one row)
-        pg.row_bytes = g.is_low ? TS_PIPE_HALF_BYTES : (16 << g.s);
-        pg.rows_half = g.is_low ? 1 : (1 << (m - 1));
-        pg.tensor = (!g.is_low && g.s <= 7) ? 1 : 0;       // box inner dimension <= 256 doubles
-        pg.box_rows = pg.rows_half < 256 ? pg.rows_half : 256;
-        pg.nbox = pg.rows_half / pg.box_rows;
+        fill_pipe_geom(g, ntiles, &pg);
         CUtensorMap tm;
         memset(&tm, 0, sizeof(tm));
         if (pg.tensor) {
             cudaError_t e = ts_tile_tensor_map(c, group, &tm);
             if (e != cudaSuccess) return e;
         }
-        pg.dbg = nullptr;
         if (getenv("TS_DEBUG")) { cudaMalloc(&pg.dbg, 64); cudaMemset(pg.dbg, 0, 64); }
         const uint64_t grid = ntiles < (uint64_t)g_num_sms ? ntiles : (uint64_t)g_num_sms;
         ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE);
@@ -424,6 +438,8 @@ bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
     if (g.g0 != TS_TILE_LOG2) return false;                            // the group right above A
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
     if (C >= c->N || C > c->chunk_max_log2) return false;
+    // mode 2 (default): only the pipelined kernel, which needs >= 512 tiles per chunk and >= 2 chunks; mode 1: ticket kernel
+    if (c->chunk_mode == 2 && (C - TS_TILE_LOG2 < 9 || c->N - C < 1)) return false;
     const int v = (ka == SW_YDAG && kb == SW_Y) ? 0 : (ka == SW_X && kb == SW_XDAG) ? 1 : -1;
     return v >= 0 && g_chunk[cfg_of(g)][v] != nullptr;
 }
@@ -433,27 +449,35 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagTables* tb
     const TileGroup& g = c->groups[gh];
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);
     const uint32_t nchunks = 1u << (c->N - C);
-    const uint32_t nblocks = 3 * nchunks;
-    if (c->sched_nchunks != nchunks) {
+    const bool piped = (c->chunk_mode == 2 && C - TS_TILE_LOG2 >= 9 && nchunks >= 2);
+    // The pipelined kernel issues the loads of a job ~1.5 tiles ahead, from a thread that still has earlier jobs to run:
+    // a dependency must lie at least one block (> 3 grid widths of jobs) back or it would wait for itself.  So its order
+    // is  P1(0) P1(1) P2(0) P2(1) P3(0) | P1(c) P3(c-1) P2(c) ...  and the last P3 runs as an ordinary pass afterwards.
+    const uint32_t nblocks = piped ? 3 * nchunks - 1 : 3 * nchunks;
+    const uint32_t key = nchunks * 2 + (piped ? 1 : 0);
+    if (c->sched_nchunks != key) {
         if (c->d_sched) cudaFree(c->d_sched);
         if (c->d_chunk_ctr) cudaFree(c->d_chunk_ctr);
         c->d_sched = nullptr; c->d_chunk_ctr = nullptr; c->sched_nchunks = 0;
         std::vector<uint32_t> sched;
-        // P1(0) P2(0) | P1(k) P3(k-1) P2(k) ... | P3(last)
-        sched.push_back(0u | (0u << 2));
-        sched.push_back(1u | (0u << 2));
-        for (uint32_t k = 1; k < nchunks; ++k) {
-            sched.push_back(0u | (k << 2));
-            sched.push_back(2u | ((k - 1) << 2));
-            sched.push_back(1u | (k << 2));
+        auto P = [](uint32_t phase, uint32_t chunk) { return phase | (chunk << 2); };
+        if (piped) {
+            sched.push_back(P(0, 0)); sched.push_back(P(0, 1)); sched.push_back(P(1, 0)); sched.push_back(P(1, 1));
+            sched.push_back(P(2, 0));
+            for (uint32_t k = 2; k < nchunks; ++k) { sched.push_back(P(0, k)); sched.push_back(P(2, k - 1)); sched.push_back(P(1, k)); }
+        } else {
+            // P1(0) P2(0) | P1(k) P3(k-1) P2(k) ... | P3(last)
+            sched.push_back(P(0, 0)); sched.push_back(P(1, 0));
+            for (uint32_t k = 1; k < nchunks; ++k) { sched.push_back(P(0, k)); sched.push_back(P(2, k - 1)); sched.push_back(P(1, k)); }
+            sched.push_back(P(2, nchunks - 1));
         }
-        sched.push_back(2u | ((nchunks - 1) << 2));
+        if (sched.size() != nblocks) return cudaErrorInvalidValue;
         cudaError_t e = cudaMalloc(&c->d_sched, sizeof(uint32_t) * nblocks);
         if (e == cudaSuccess) e = cudaMalloc(&c->d_chunk_ctr, sizeof(unsigned int) * (64 + 2 * (size_t)nchunks));
         if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_sched, sched.data(), sizeof(uint32_t) * nblocks, cudaMemcpyHostToDevice, c->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);    // `sched` is a temporary
         if (e != cudaSuccess) return e;
-        c->sched_nchunks = nchunks;
+        c->sched_nchunks = key;
     }
     ChunkParams q;
     fill_params(c, g, nullptr, &q.h);
@@ -465,8 +489,28 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagTables* tb
     cudaError_t e = cudaMemsetAsync(c->d_chunk_ctr, 0, sizeof(unsigned int) * (64 + 2 * (size_t)nchunks), c->stream);
     if (e != cudaSuccess) return e;
     const int v = (ka == SW_YDAG) ? 0 : 1;
-    chunk_kernel_t k = g_chunk[cfg_of(g)][v];
     const uint64_t jobs = (uint64_t)nblocks << q.tiles_log2;
+    if (piped) {
+        PipeGeom pg;
+        fill_pipe_geom(g, jobs, &pg);
+        CUtensorMap tm;
+        memset(&tm, 0, sizeof(tm));
+        if (pg.tensor) {
+            e = ts_tile_tensor_map(c, gh, &tm);
+            if (e != cudaSuccess) return e;
+        }
+        const uint64_t grid1 = jobs < (uint64_t)g_num_sms ? jobs : (uint64_t)g_num_sms;
+        ts_prof_begin(c, TS_KC_TILE_CHUNK);
+        // cooperative launch: the CTAs wait on one another's progress, so they must all be resident (else: error, not a hang)
+        void* args[3] = {(void*)&q, (void*)&tm, (void*)&pg};
+        e = cudaLaunchCooperativeKernel((const void*)g_chunk_pipe[cfg_of(g)][v], dim3((unsigned)grid1), dim3(TS_PIPE_THREADS), args,
+                                        TS_PIPE_SMEM, c->stream);
+        ts_prof_end(c);
+        if (e != cudaSuccess) return e;
+        // the last chunk's third phase
+        return ts_tile_pass(c, gh, kb, nullptr, SW_NONE, (uint64_t)(nchunks - 1) << q.tiles_log2, (uint64_t)1 << q.tiles_log2);
+    }
+    chunk_kernel_t k = g_chunk[cfg_of(g)][v];
     uint64_t grid = 2 * (uint64_t)g_num_sms;
     if (grid > jobs) grid = jobs;
     ts_prof_begin(c, TS_KC_TILE_CHUNK);

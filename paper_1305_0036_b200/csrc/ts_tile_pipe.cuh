@@ -33,6 +33,7 @@ struct PipeGeom {
     int rows_half;        // rows per half tile
     int row_bytes;        // 16 << s
     int box_rows, nbox;   // tensor mode: boxes per half tile
+    int pf;               // L2 prefetch distance in half tiles (0 = off): TMA prefetches into L2 cost no shared memory
     unsigned long long* dbg;   // TS_DEBUG: [0] mismatches between landed halves and direct global reads, [1..4] first one
 };
 
@@ -84,6 +85,15 @@ __device__ __forceinline__ void tensor_load_3d(uint32_t dst, const CUtensorMap* 
         "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
 }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tensor_prefetch_l2_3d(const CUtensorMap* tm, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tm), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
 __device__ __forceinline__ void group_sync(int grp)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(TS_TILE_THREADS) : "memory");
@@ -105,6 +115,101 @@ __device__ __forceinline__ void exchange_g(double2* sm, double (&re)[32], double
         const double2 v = sm[slot_of(f)];
         re[r] = v.x; im[r] = v.y;
     }
+}
+
+// Sweeps, diagonal and in-place store of one tile held in registers in layout 1 (used by k_tile_pipe and k_chunk_pipe).
+// STCG: keep the stored lines in L2 (st.global.cg) instead of streaming them out (st.global.cs).
+template <int K1, int K2, int BF1, int BF2, int NSHFL, bool STCG>
+__device__ __forceinline__ void pipe_compute_store(const TilePassParams& p, const uint64_t tau, double (&re)[32], double (&im)[32],
+                                                   const double2 base, const double2 (&w)[5], double2* E, const int t, const int grp)
+{
+    constexpr bool GENERIC = (BF1 < 0);
+    const bool two_stage = GENERIC ? (p.two_stage != 0) : (BF2 != 0);
+    const int nshfl = GENERIC ? p.nshfl : NSHFL;
+    const int lane = t & 31;
+    const bool has_diag = (p.tile_phase != nullptr);
+    const int s = p.s, g0 = p.g0, nmid = g0 - s;
+    const uint64_t runmask = ((uint64_t)1 << s) - 1;
+    const uint64_t base_idx = ((tau & (((uint64_t)1 << nmid) - 1)) << s) | ((tau >> nmid) << (g0 + TS_TILE_LOG2 - s));
+
+    // Single sweep of a high group with runs of >= 8 amplitudes and no diagonal: ONE exchange.  Layout 2H keeps the run
+    // bits f0..2 on the lanes (f = (t & 7) | r << 3 | (t >> 3) << 8; registers hold f3..7), so the tile can be stored
+    // straight from it in full 128-byte runs, exactly as coalesced as from layout 1.
+    if (K2 == SW_NONE && NSHFL == 0 && !GENERIC && BF2 != 0 && (BF2 & 1) == 0 && !has_diag) {
+        bfly_regs<K1, BF1>(re, im, p.bf1);
+#pragma unroll
+        for (int r = 0; r < 32; ++r) E[slot_of(f_layout1(t, r))] = make_double2(re[r], im[r]);
+        group_sync(grp);
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            const double2 v = E[slot_of((t & 7) | (r << 3) | ((t >> 3) << 8))];
+            re[r] = v.x; im[r] = v.y;
+        }
+        bfly_regs<K1, ((BF2 >= 0 ? BF2 : 0) >> 1)>(re, im, 0u);          // f3..6 sit on register bits 0..3 here
+        uint64_t ob[5];
+#pragma unroll
+        for (int b = 0; b < 5; ++b) {
+            const uint64_t f = (uint64_t)1 << (3 + b);
+            ob[b] = (f & runmask) | ((f >> s) << g0);
+        }
+        const uint64_t ft = (uint64_t)((t & 7) | ((t >> 3) << 8));
+        double2* __restrict__ gq = p.psi + base_idx + ((ft & runmask) | ((ft >> s) << g0));
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            uint64_t o = 0;
+#pragma unroll
+            for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= ob[b];
+            if (STCG) __stcg(gq + o, make_double2(re[r], im[r]));
+            else __stcs(gq + o, make_double2(re[r], im[r]));
+        }
+        return;      // (the two barriers of the next tile's landing reads separate these reads of E from its next writes)
+    }
+
+    // ---- sweep K1
+    bfly_regs<K1, BF1>(re, im, p.bf1);
+    if (two_stage) {
+        exchange_g<true>(E, re, im, t, grp);
+        bfly_regs<K1, BF2>(re, im, p.bf2);
+        if (nshfl) { bfly_lane<K1>(re, im, 0, lane); bfly_lane<K1>(re, im, 1, lane); }
+    }
+    // ---- diagonal
+    if (has_diag) apply_diag(p, base, w, re, im);
+    // ---- sweep K2 (mirror order)
+    if (two_stage) {
+        if (nshfl) { bfly_lane<K2>(re, im, 1, lane); bfly_lane<K2>(re, im, 0, lane); }
+        bfly_regs<K2, BF2>(re, im, p.bf2);
+        exchange_g<false>(E, re, im, t, grp);
+    }
+    bfly_regs<K2, BF1>(re, im, p.bf1);
+
+    // global element offset of in-tile index f: run bits stay, group bits move up to g0
+    uint64_t offb[5];
+#pragma unroll
+    for (int b = 0; b < 5; ++b) {
+        const uint64_t f = (uint64_t)1 << (7 + b);
+        offb[b] = (f & runmask) | ((f >> s) << g0);
+    }
+    const uint64_t offt = ((uint64_t)t & runmask) | (((uint64_t)t >> s) << g0);
+    double2* __restrict__ gp = p.psi + base_idx + offt;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+        uint64_t o = 0;
+#pragma unroll
+        for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
+        if (STCG) __stcg(gp + o, make_double2(re[r], im[r]));
+        else __stcs(gp + o, make_double2(re[r], im[r]));
+    }
+}
+
+// Per-thread phase factors from the tile-phase record `tp` (32 entries, in shared memory) and the thread tables.
+__device__ __forceinline__ void pipe_thread_phase(const TilePassParams& p, const double2* tp, const int t, double2& base, double2 (&w)[5])
+{
+    base = cmul(tp[0], __ldg(p.TT + t));
+    base = cmul(base, tp[1 + (t & 15)]);
+    base = cunit(cmul(base, tp[17 + (t >> 4)]));
+    base.x *= p.scale; base.y *= p.scale;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) w[k] = cunit(cmul(tp[25 + k], __ldg(p.WT + k * 128 + t)));
 }
 
 template <int K1, int K2, int BF1, int BF2, int NSHFL>
@@ -137,7 +242,26 @@ k_tile_pipe(const __grid_constant__ TilePassParams p, const __grid_constant__ CU
     const uint64_t n_cta = (g.ntiles > blockIdx.x) ? (g.ntiles - blockIdx.x + G - 1) / G : 0;
     const uint64_t n_half = 2 * n_cta;
 
+    // half q of this CTA into L2 only (the ring holds 1.5 tiles, not enough bytes in flight to cover HBM latency)
+    auto prefetch_half = [&](uint64_t q) {
+        const uint64_t tau = p.tile_base + blockIdx.x + (q >> 1) * G;
+        const int h = (int)(q & 1);
+        const uint64_t mid = tau & midmask, hi = tau >> nmid;
+        if (g.tensor) {
+            for (int b = 0; b < g.nbox; ++b)
+                tensor_prefetch_l2_3d(&tmap, (int)(mid << (s + 1)), h * g.rows_half + b * g.box_rows, (int)hi);
+        } else {
+            const uint64_t base_idx = (mid << s) | (hi << (g0 + TS_TILE_LOG2 - s));
+            if (g.is_low) {
+                bulk_prefetch_l2(p.psi + base_idx + (uint64_t)h * (TS_PIPE_HALF_BYTES / 16), TS_PIPE_HALF_BYTES);
+            } else {
+                for (int r = 0; r < g.rows_half; ++r)
+                    bulk_prefetch_l2(p.psi + base_idx + ((uint64_t)(h * g.rows_half + r) << g0), g.row_bytes);
+            }
+        }
+    };
     auto issue_load = [&](uint64_t q, int slot) {
+        if (g.pf > 0 && q + g.pf < n_half) prefetch_half(q + g.pf);
         const uint64_t i = q >> 1;
         const int h = (int)(q & 1);
         const uint64_t tau = p.tile_base + blockIdx.x + i * G;
@@ -168,6 +292,7 @@ k_tile_pipe(const __grid_constant__ TilePassParams p, const __grid_constant__ CU
         cons[0] = 0; cons[1] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        for (uint64_t q = TS_PIPE_SLOTS; q < (uint64_t)(TS_PIPE_SLOTS + g.pf) && q < n_half; ++q) prefetch_half(q);
         for (uint64_t q = 0; q < TS_PIPE_SLOTS && q < n_half; ++q) issue_load(q, (int)q);
     }
     __syncthreads();
@@ -215,13 +340,7 @@ k_tile_pipe(const __grid_constant__ TilePassParams p, const __grid_constant__ CU
                 }
             }
             if (h == 0 && has_diag) {
-                const double2* tp = TPs + slot * 32;
-                base = cmul(tp[0], __ldg(p.TT + t));
-                base = cmul(base, tp[1 + (t & 15)]);
-                base = cunit(cmul(base, tp[17 + (t >> 4)]));
-                base.x *= p.scale; base.y *= p.scale;
-#pragma unroll
-                for (int k = 0; k < 5; ++k) w[k] = cunit(cmul(tp[25 + k], __ldg(p.WT + k * 128 + t)));
+                pipe_thread_phase(p, TPs + slot * 32, t, base, w);
             }
             group_sync(grp);
             if (t == 0) {
@@ -235,32 +354,7 @@ k_tile_pipe(const __grid_constant__ TilePassParams p, const __grid_constant__ CU
         // skip the other group's two halves
         slot += 2; if (slot >= TS_PIPE_SLOTS) { slot -= TS_PIPE_SLOTS; use += 1; }
 
-        // ---- sweep K1
-        bfly_regs<K1, BF1>(re, im, p.bf1);
-        if (two_stage) {
-            exchange_g<true>(E, re, im, t, grp);
-            bfly_regs<K1, BF2>(re, im, p.bf2);
-            if (nshfl) { bfly_lane<K1>(re, im, 0, lane); bfly_lane<K1>(re, im, 1, lane); }
-        }
-        // ---- diagonal
-        if (has_diag) apply_diag(p, base, w, re, im);
-        // ---- sweep K2 (mirror order)
-        if (two_stage) {
-            if (nshfl) { bfly_lane<K2>(re, im, 1, lane); bfly_lane<K2>(re, im, 0, lane); }
-            bfly_regs<K2, BF2>(re, im, p.bf2);
-            exchange_g<false>(E, re, im, t, grp);
-        }
-        bfly_regs<K2, BF1>(re, im, p.bf1);
-
-        const uint64_t base_idx = ((tau & midmask) << s) | ((tau >> nmid) << (g0 + TS_TILE_LOG2 - s));
-        double2* __restrict__ gp = p.psi + base_idx + offt;
-#pragma unroll
-        for (int r = 0; r < 32; ++r) {
-            uint64_t o = 0;
-#pragma unroll
-            for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
-            __stcs(gp + o, make_double2(re[r], im[r]));
-        }
+        pipe_compute_store<K1, K2, BF1, BF2, NSHFL, false>(p, tau, re, im, base, w, E, t, grp);
     }
 }
 
