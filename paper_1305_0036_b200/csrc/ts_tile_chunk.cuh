@@ -103,23 +103,46 @@ k_chunk_pipe(const __grid_constant__ ChunkParams q, const __grid_constant__ CUte
     const uint64_t n_half = 2 * n_cta;
     const bool a_diag = (q.a.tile_phase != nullptr);
 
+    // job i of this CTA -> (phase, chunk, tile); the block order of ts_tile.cu's pipelined schedule in closed form
+    // (P1(0) P1(1) P2(0) P2(1) P3(0) | P1(c) P3(c-1) P2(c), c >= 2): no table read on the issuing thread's critical path
     auto job_of = [&](uint64_t i, uint32_t& phase, uint32_t& c, uint64_t& tau) {
         const uint64_t n = blockIdx.x + i * G;
-        const uint32_t e = __ldg(q.sched + (n >> tl));
-        phase = e & 3u; c = e >> 2;
+        const uint32_t B = (uint32_t)(n >> tl);
+        if (B < 5) { phase = (B < 2) ? 0u : (B < 4 ? 1u : 2u); c = (B == 1 || B == 3) ? 1u : 0u; }
+        else {
+            const uint32_t k = B - 5, r = k % 3;
+            c = 2 + k / 3;
+            if (r == 0) phase = 0; else if (r == 1) { phase = 2; c -= 1; } else phase = 1;
+        }
         tau = ((uint64_t)c << tl) | (n & (T - 1));
     };
-    uint32_t ok_dep = 0xffffffffu;           // (phase << 28 | chunk) whose dependency this thread last saw satisfied
+    auto dep_ptr = [&](uint32_t phase, uint32_t c) { return q.done + (size_t)(phase - 1) * q.nchunks + c; };
+    // issuing-thread state lives in shared memory (only thread 0 of each group touches it): registers are all taken
+    // st[0] = ok_dep: (phase << 28 | chunk) whose dependency this thread last saw satisfied; st[1], st[2] = pre_key,
+    // pre_val: counter value read ahead of time for the job issued next; st[3] = pending publish (index + 1 into done)
+    volatile uint32_t* st = reinterpret_cast<volatile uint32_t*>(smraw + TS_PIPE_OFF_BAR + 40) + 4 * grp;
+#define ok_dep st[0]
+#define pre_key st[1]
+#define pre_val st[2]
     auto issue_load = [&](uint64_t qh, int slot) {
         uint32_t phase, c; uint64_t tau;
         job_of(qh >> 1, phase, c, tau);
         const int h = (int)(qh & 1);
-        if (phase != 0 && ok_dep != ((phase << 28) | c)) {
-            const volatile unsigned int* d = q.done + (size_t)(phase - 1) * q.nchunks + c;
-            while (*d < T) __nanosleep(100);
+        const uint32_t key = (phase << 28) | c;
+        if (phase != 0 && ok_dep != key) {
+            if (!(pre_key == key && pre_val >= T)) {
+                const volatile unsigned int* d = dep_ptr(phase, c);
+                while (*d < T) __nanosleep(100);
+            }
             __threadfence();
             asm volatile("fence.proxy.async;" ::: "memory");     // the TMA engine reads what other SMs' threads wrote
-            ok_dep = (phase << 28) | c;
+            ok_dep = key;
+        }
+        {   // read the next job's dependency counter now; it is looked at when that job's load is issued
+            uint32_t p2, c2; uint64_t t2;
+            job_of((qh >> 1) + 1, p2, c2, t2);
+            const uint32_t k2 = (p2 << 28) | c2;
+            if (p2 != 0 && k2 != ok_dep && (qh >> 1) + 1 < n_cta) { pre_key = k2; pre_val = *(const volatile unsigned int*)dep_ptr(p2, c2); }
         }
         const uint32_t bar = sBar + 8 * slot;
         const uint32_t dst = sL + slot * TS_PIPE_HALF_BYTES;
@@ -147,6 +170,7 @@ k_chunk_pipe(const __grid_constant__ ChunkParams q, const __grid_constant__ CUte
     if (threadIdx.x == 0) {
         for (int k = 0; k < TS_PIPE_SLOTS; ++k) mbar_init(sBar + 8 * k, 1);
         cons[0] = 0; cons[1] = 0;
+        for (int k = 0; k < 8; ++k) (reinterpret_cast<volatile uint32_t*>(smraw + TS_PIPE_OFF_BAR + 40))[k] = (k & 3) < 2 ? 0xffffffffu : 0u;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         for (uint64_t qh = 0; qh < TS_PIPE_SLOTS && qh < n_half; ++qh) issue_load(qh, (int)qh);
@@ -154,7 +178,6 @@ k_chunk_pipe(const __grid_constant__ ChunkParams q, const __grid_constant__ CUte
     __syncthreads();
 
     uint32_t slot = (2 * grp) % TS_PIPE_SLOTS, use = (2 * grp) / TS_PIPE_SLOTS;
-    unsigned int* pending = nullptr;          // done counter of this group's previous tile, published late (see below)
 
     for (uint64_t i = grp; i < n_cta; i += 2) {
         uint32_t phase, c; uint64_t tau;
@@ -176,7 +199,7 @@ k_chunk_pipe(const __grid_constant__ ChunkParams q, const __grid_constant__ CUte
             if (t == 0) {
                 // every thread of the group issued the stores of the previous tile before this barrier: publish it now
                 // (the fence is cumulative over the barrier), off the critical path of that tile
-                if (h == 0 && pending) { __threadfence(); atomicAdd(pending, 1u); pending = nullptr; }
+                if (h == 0 && st[3]) { __threadfence(); atomicAdd(q.done + (st[3] - 1), 1u); st[3] = 0; }
                 const uint64_t qn = 2 * i + h + TS_PIPE_SLOTS;
                 if (qn < n_half) issue_load(qn, (int)slot);
                 if (h == 0) cons[grp] = (uint32_t)i + 1;
@@ -188,10 +211,13 @@ k_chunk_pipe(const __grid_constant__ ChunkParams q, const __grid_constant__ CUte
         if (phase == 0) pipe_compute_store<KA, SW_NONE, HBF1, HBF2, 0, true>(q.h, tau, re, im, base, w, E, t, grp);
         else if (phase == 1) pipe_compute_store<KA, KB, 31, 31, 2, true>(q.a, tau, re, im, base, w, E, t, grp);
         else pipe_compute_store<KB, SW_NONE, HBF1, HBF2, 0, false>(q.h, tau, re, im, base, w, E, t, grp);
-        if (t == 0 && phase != 2) pending = q.done + (size_t)phase * q.nchunks + c;
+        if (t == 0 && phase != 2) st[3] = phase * q.nchunks + c + 1;
     }
     group_sync(grp);
-    if (t == 0 && pending) { __threadfence(); atomicAdd(pending, 1u); }
+    if (t == 0 && st[3]) { __threadfence(); atomicAdd(q.done + (st[3] - 1), 1u); }
+#undef ok_dep
+#undef pre_key
+#undef pre_val
 }
 
 #define TS_CHUNK_REGISTER_CFG(NAME, BF1, BF2)                                                                     \

@@ -24,7 +24,7 @@
 #define TS_PIPE_OFF_E (TS_PIPE_SLOTS * TS_PIPE_HALF_BYTES)
 #define TS_PIPE_OFF_TP (TS_PIPE_OFF_E + 2 * 65536)
 #define TS_PIPE_OFF_BAR (TS_PIPE_OFF_TP + TS_PIPE_SLOTS * 512)
-#define TS_PIPE_SMEM (TS_PIPE_OFF_BAR + 64)
+#define TS_PIPE_SMEM (TS_PIPE_OFF_BAR + 128)
 
 struct PipeGeom {
     uint64_t ntiles;      // tiles of this launch
