@@ -251,8 +251,17 @@ def run_ours(args):
     round_trips = prof["tile_fused"]["launches"] + prof["tile_single"]["launches"] + prof["tile_chunk3"]["launches"]
     tile_passes = prof["tile_fused"]["launches"] + prof["tile_single"]["launches"] + 3 * prof["tile_chunk3"]["launches"]
     step_ms = ms / args.steps
+    traffic = None                    # dram__bytes_read + write of the dominant kernel from the committed ncu capture (N = 30)
+    try:                              # (values and the command that produced them: profiles/r01b_pipeline_and_l2_blocking.md)
+        with open(os.path.join(ROOT, "profiles", "r01b_traffic.csv")) as f:
+            for line in f.read().splitlines()[1:]:
+                k, rd, wr = line.split(",")
+                if N == 30 and k == dom:
+                    traffic = float(rd) + float(wr)
+    except Exception:
+        traffic = None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic,
                 "alg_bytes_per_launch": alg_bytes, "tile_passes_per_launch": passes_per_launch[dom],
                 "hbm_round_trip_bytes_per_launch": pass_bytes, "avg_launch_ms": dms,
                 "step_gbs_over_tile_passes": tile_passes * pass_bytes / (ms * 1e-3) / 1e9,
