@@ -178,3 +178,13 @@ def test_config5_grid32_properties(B):
     assert np.max(np.abs(ts.expect_all(B.Z) - sz0)) <= OBS_TOL
     assert abs(ts.norm2() - 1.0) <= 1e-12
     ts.close()
+
+
+@pytest.mark.parametrize("pipe,chunk3", [(0, 0), (2, 0), (1, 1)])
+def test_kernel_variants_N26(B, pipe, chunk3, monkeypatch):
+    """The execution switches read at ts_create: first kernel only (TS_PIPE=0), pipelined kernel for
+    every tile pass (TS_PIPE=2), ticket-scheduled L2-blocked triple launch (TS_CHUNK3=1).  Same gate as the default
+    path, which the other tests of this file run (pipelined fused passes + pipelined triple launch at N = 30)."""
+    monkeypatch.setenv("TS_PIPE", str(pipe))
+    monkeypatch.setenv("TS_CHUNK3", str(chunk3))
+    check_clustered(B, 26, 3, 1, seed=2600 + 10 * pipe + chunk3, n_windows=32)
