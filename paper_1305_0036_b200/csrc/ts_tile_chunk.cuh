@@ -196,7 +196,7 @@ k_chunk_pipe(const __grid_constant__ ChunkParams q, const __grid_constant__ CUte
             }
             if (h == 0 && phase == 1 && a_diag) pipe_thread_phase(q.a, TPs + slot * 32, t, base, w);
             group_sync(grp);
-            if (t == 0) {
+            if (t == (h ? 32 : 0)) {     // the two halves are served by different warps: neither is late twice
                 // every thread of the group issued the stores of the previous tile before this barrier: publish it now
                 // (the fence is cumulative over the barrier), off the critical path of that tile
                 if (h == 0 && st[3]) { __threadfence(); atomicAdd(q.done + (st[3] - 1), 1u); st[3] = 0; }

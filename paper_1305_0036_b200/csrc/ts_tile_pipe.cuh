@@ -343,7 +343,7 @@ k_tile_pipe(const __grid_constant__ TilePassParams p, const __grid_constant__ CU
                 pipe_thread_phase(p, TPs + slot * 32, t, base, w);
             }
             group_sync(grp);
-            if (t == 0) {
+            if (t == (h ? 32 : 0)) {     // the two halves are served by different warps: neither is late twice
                 const uint64_t qn = 2 * i + h + TS_PIPE_SLOTS;
                 if (qn < n_half) issue_load(qn, (int)slot);
                 if (h == 0) cons[grp] = (uint32_t)i + 1;
