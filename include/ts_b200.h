@@ -87,6 +87,14 @@ int ts_get_state(ts_ctx* ctx, void* dst, uint64_t first, uint64_t count, int whe
  * TS_ERR_NOSTATE, TS_ERR_CUDA. */
 int ts_evolve(ts_ctx* ctx, double tau, int64_t n_steps, int order);
 
+/* n_steps single steps U_order(tau), recording an observable after EVERY step (magnitudes followed in time;
+ * BASELINE config 2 records <S^z_1>(t)) without a host round trip per step: the reductions write rows of a device
+ * trace, copied once at the end.  alpha = TS_Z, j = -1: out[n_steps][N] = <S^z_s> of all sites; alpha = TS_Z, j >= 0:
+ * out[n_steps]; alpha = TS_X / TS_Y: one site j, out[n_steps].  Steps are applied one by one (the state after each
+ * step is needed), so the diagonals at step boundaries are not merged: round-off differs from ts_evolve(tau, n_steps)
+ * at the 1e-15 level.  Synchronises at the end.  Errors: as ts_evolve, TS_ERR_NOMEM. */
+int ts_evolve_observe(ts_ctx* ctx, double tau, int64_t n_steps, int order, int alpha, int j, double* out);
+
 /* out[0] = <psi|S^alpha_j|psi>, j 0-based (reading A15).  Synchronises. */
 int ts_expect(ts_ctx* ctx, int alpha, int j, double* out);
 

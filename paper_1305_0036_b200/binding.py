@@ -23,7 +23,7 @@ KC_COUNT = len(KC_NAMES)
 
 # every symbol include/ts_b200.h declares (tests check that the library exports all of them)
 SYMBOLS = ("ts_create", "ts_destroy", "ts_set_stream", "ts_bind_state", "ts_set_state", "ts_set_basis_state",
-           "ts_set_state_range", "ts_get_state", "ts_evolve", "ts_expect", "ts_expect_all", "ts_norm2", "ts_overlap", "ts_set_plan",
+           "ts_set_state_range", "ts_get_state", "ts_evolve", "ts_evolve_observe", "ts_expect", "ts_expect_all", "ts_norm2", "ts_overlap", "ts_set_plan",
            "ts_describe_plan", "ts_set_profiling", "ts_get_profile", "ts_reset_profile", "ts_strerror", "ts_version")
 
 _lib = None
@@ -56,6 +56,7 @@ def load() -> ctypes.CDLL:
         "ts_set_basis_state": (I, [_vp, U64]),
         "ts_get_state": (I, [_vp, _vp, U64, U64, I]),
         "ts_evolve": (I, [_vp, D, I64, I]),
+        "ts_evolve_observe": (I, [_vp, D, I64, I, I, I, _dp]),
         "ts_expect": (I, [_vp, I, I, _dp]),
         "ts_expect_all": (I, [_vp, I, _dp]),
         "ts_norm2": (I, [_vp, _dp]),
@@ -190,6 +191,14 @@ class TrotterSuzuki:
     # ------------------------------------------------------------------ the hot path
     def evolve(self, tau: float, n_steps: int, order: int = 4):
         _check(self._lib.ts_evolve(self._ctx, float(tau), int(n_steps), int(order)), "ts_evolve")
+
+    def evolve_observe(self, tau: float, n_steps: int, order: int = 4, alpha: int = Z, j: int = -1) -> np.ndarray:
+        """n_steps steps, the observable after every step: [n_steps][N] for alpha = Z, j = -1, else [n_steps]."""
+        shape = (n_steps, self.N) if (alpha == Z and j < 0) else (n_steps,)
+        out = np.zeros(shape)
+        _check(self._lib.ts_evolve_observe(self._ctx, float(tau), int(n_steps), int(order), int(alpha), int(j),
+                                           out.ctypes.data_as(_dp)), "ts_evolve_observe")
+        return out
 
     def expect(self, alpha: int, j: int) -> float:
         out = ctypes.c_double()

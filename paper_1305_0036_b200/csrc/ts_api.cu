@@ -404,6 +404,43 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
     return cuda_status(e);
 }
 
+int ts_evolve_observe(ts_ctx* c, double tau, int64_t n_steps, int order, int alpha, int j, double* out)
+{
+    if (!c || !out || !isfinite(tau) || n_steps < 0 || (order != 2 && order != 4) || alpha < TS_X || alpha > TS_Z) return TS_ERR_ARG;
+    if (alpha == TS_Z ? (j < -1 || j >= c->N) : (j < 0 || j >= c->N)) return TS_ERR_ARG;
+    if (!c->psi) return TS_ERR_NOSTATE;
+    if (n_steps == 0) return TS_OK;
+    double* d_trace = nullptr;
+    cudaError_t e = cudaMalloc(&d_trace, sizeof(double) * TS_TRACE_STRIDE * (size_t)n_steps);
+    if (e != cudaSuccess) { cudaGetLastError(); return TS_ERR_NOMEM; }
+    int st = TS_OK;
+    for (int64_t k = 0; k < n_steps && st == TS_OK; ++k) {
+        st = ts_evolve(c, tau, 1, order);
+        if (st == TS_OK) st = cuda_status(ts_reduce_trace_row(c, alpha, j < 0 ? 0 : j, d_trace + (size_t)k * TS_TRACE_STRIDE));
+    }
+    std::vector<double> host;
+    if (st == TS_OK) {
+        host.resize((size_t)TS_TRACE_STRIDE * n_steps);
+        e = cudaMemcpyAsync(host.data(), d_trace, sizeof(double) * host.size(), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        st = cuda_status(e);
+    } else {
+        cudaStreamSynchronize(c->stream);
+    }
+    cudaFree(d_trace);
+    if (st != TS_OK) return st;
+    for (int64_t k = 0; k < n_steps; ++k) {
+        const double* row = host.data() + (size_t)k * TS_TRACE_STRIDE;
+        if (alpha == TS_Z) {
+            if (j < 0) for (int s = 0; s < c->N; ++s) out[(size_t)k * c->N + s] = row[1 + s] - 0.5 * row[0];
+            else out[k] = row[1 + j] - 0.5 * row[0];
+        } else {
+            out[k] = (alpha == TS_X) ? row[0] : row[1];
+        }
+    }
+    return TS_OK;
+}
+
 int ts_expect(ts_ctx* c, int alpha, int j, double* out)
 {
     if (!c || !out || alpha < TS_X || alpha > TS_Z || j < 0 || j >= c->N) return TS_ERR_ARG;

@@ -115,3 +115,5 @@ cudaError_t ts_reduce_expect_xy(ts_ctx* c, int alpha, int j, double* out_host);
 cudaError_t ts_reduce_norm2(ts_ctx* c, double* out_host);
 cudaError_t ts_reduce_overlap(ts_ctx* c, const double2* phi, double* out_host /*[2]*/);
 cudaError_t ts_fill_basis(ts_ctx* c, uint64_t k);
+#define TS_TRACE_STRIDE (TS_MAX_N + 1)
+cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row /*[TS_TRACE_STRIDE]*/);

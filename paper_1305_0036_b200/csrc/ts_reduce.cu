@@ -148,7 +148,38 @@ cudaError_t finish(ts_ctx* c, int grid, int nvals, double* host_out)
     return cudaStreamSynchronize(c->stream);
 }
 
+// final sum of nvals values into a DEVICE buffer, no copy, no synchronisation (observable traces)
+cudaError_t finish_dev(ts_ctx* c, int grid, int nvals, double* dev_out)
+{
+    k_final_sum<<<1, 64, 0, c->stream>>>(c->d_red, grid, nvals, dev_out);
+    ts_prof_end(c);
+    return cudaGetLastError();
+}
+
 } // namespace
+
+// One row of an observable trace, written to device memory on the stream (ts_evolve_observe):
+// alpha = z: row[0] = <psi|psi>, row[1 + j] = sum_{k: bit j = 1} |c_k|^2 for all j;  alpha = x, y: row[0], row[1] = the
+// Re and Im pair sums of site j.  The host turns rows into expectation values after the single final copy.
+cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row)
+{
+    if (alpha == TS_Z) {
+        const uint64_t dim = (uint64_t)1 << c->N;
+        const int grid = red_grid(dim);
+        cudaError_t e = ensure_scratch(c, (size_t)(grid + 1) * MAXV);
+        if (e != cudaSuccess) return e;
+        ts_prof_begin(c, TS_KC_REDUCE);
+        k_prob_bits<<<grid, RB, 0, c->stream>>>(c->psi, c->N, dim, c->d_red);
+        return finish_dev(c, grid, c->N + 1, dev_row);
+    }
+    const uint64_t npairs = (uint64_t)1 << (c->N - 1);
+    const int grid = red_grid(npairs);
+    cudaError_t e = ensure_scratch(c, (size_t)(grid + 1) * MAXV);
+    if (e != cudaSuccess) return e;
+    ts_prof_begin(c, TS_KC_REDUCE);
+    k_pair_xy<<<grid, RB, 0, c->stream>>>(c->psi, j, npairs, c->d_red);
+    return finish_dev(c, grid, 2, dev_row);
+}
 
 cudaError_t ts_reduce_expect_z_all(ts_ctx* c, double* out_host)
 {

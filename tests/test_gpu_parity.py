@@ -167,3 +167,32 @@ def test_config3_dipolar22(B):
     check_amps(ts.get_state(), ref)
     got = ts.expect_all(2)
     assert np.max(np.abs(got - O.expect_all(ref, w.N, 2))) <= OBS_TOL
+
+
+def test_config2_trace_without_host_round_trips(B):
+    """ts_evolve_observe: the same <S^z_1>(t) trace as above from one call (device-side trace, one copy at the end),
+    plus all-site and x / y traces of a few steps against the oracle."""
+    w = W.config(2)
+    ts = B.TrotterSuzuki(w.N, w.h, w.J)
+    ts.set_basis_state(w.basis_index)
+    got = ts.evolve_observe(w.tau, w.n_steps, 4, B.Z, 0)
+    psi = w.state()
+    ref = []
+    for _ in range(w.n_steps):
+        O.evolve(psi, w.N, w.h, w.J, w.tau, 1, 4, True)
+        ref.append(O.expect(psi, w.N, 2, 0))
+    assert got.shape == (w.n_steps,)
+    assert np.max(np.abs(got - np.array(ref))) <= OBS_TOL
+    check_amps(ts.get_state(), psi)
+    ts.set_basis_state(w.basis_index)
+    allz = ts.evolve_observe(w.tau, 3, 4, B.Z, -1)
+    ts.set_basis_state(w.basis_index)
+    sx = ts.evolve_observe(w.tau, 3, 4, B.X, 5)
+    ts.set_basis_state(w.basis_index)
+    sy = ts.evolve_observe(w.tau, 3, 4, B.Y, 5)
+    psi = w.state()
+    for k in range(3):
+        O.evolve(psi, w.N, w.h, w.J, w.tau, 1, 4, True)
+        assert np.max(np.abs(allz[k] - O.expect_all(psi, w.N, 2))) <= OBS_TOL
+        assert abs(sx[k] - O.expect(psi, w.N, 0, 5)) <= OBS_TOL
+        assert abs(sy[k] - O.expect(psi, w.N, 1, 5)) <= OBS_TOL
