@@ -31,7 +31,11 @@ UNIT = "steps/s"
 N_SWEEPS_PER_STEP = 20
 
 
-def workload_for(N: int) -> W.Workload:
+def workload_for(N: int, kind: str = "grid") -> W.Workload:
+    if kind == "chain":          # Heisenberg chain, random z fields (config-1 recipe at size N)
+        return W.chain_like(N, seed=8, tau=0.01, n_steps=5)
+    if kind == "dipolar":        # all-to-all dipolar network, random product state (config-3 recipe at size N)
+        return W.dipolar_like(N, seed=8, tau=0.005, n_steps=5)
     if N == 30:
         return W.config("M")
     return W.grid_like(N, seed=8, tau=0.01, n_steps=5, state_seed=9, cols=6 if N >= 24 else None)
@@ -169,7 +173,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     N = args.N
-    w = workload_for(N)
+    w = workload_for(N, args.workload)
     if world > 1:                      # independent ensemble members: same Hamiltonian, different random state
         w.state_seed = R.replica_state_seed(w.state_seed, rank)
     dim = 1 << N
@@ -270,7 +274,7 @@ def run_ours(args):
                                                 * pass_bytes / 8e12) / (step_ms * 1e-3)}
     cpu = None
     if not args.no_cpu:
-        s = oracle_sample(N, workload_for(N))
+        s = oracle_sample(N, workload_for(N))      # (always the lattice recipe: the oracle's cost does not depend on it)
         cpu = {"value": s["value"], "unit": UNIT, "cores": s["cores"], "kind": "oracle", "sample": s["sample"],
                "sample_steps_per_s": s["steps_per_s_sample"]}
 
@@ -297,6 +301,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--N", type=int, default=30)
+    ap.add_argument("--workload", default="grid", choices=["grid", "chain", "dipolar"],
+                    help="Hamiltonian family (north_star: chains, lattices, all-to-all); the metric line is the default grid")
     ap.add_argument("--plan", default="", help="mode,run_bits,max_group_bits (ts_set_plan)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
