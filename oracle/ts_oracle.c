@@ -331,3 +331,101 @@ void tso_overlap(const double *phi, const double *psi, int N, double *out)
     }
     out[0] = sr; out[1] = si;
 }
+
+/* ------------------------------------------------------------------------------------------------------------
+ * "Local and non-local physical magnitudes" beyond the one-site expectation values; the paper names them
+ * without formulas, so these are the textbook definitions in the conventions of the header (reading A15):
+ *
+ * Two-site correlator <psi| S^a_j S^a_k |psi>, j != k, un-normalised.  With m = 2^j + 2^k and sigma = bit - 1/2:
+ *   zz:  sum_i sigma_j(i) sigma_k(i) |c_i|^2
+ *   xx:  1/4 sum_i conj(c_{i xor m}) c_i                         (S^x = 1/2 (|up><down| + |down><up|) flips the bit)
+ *   yy: -sum_i sigma_j(i) sigma_k(i) conj(c_{i xor m}) c_i       (S^y|up> = i/2 |down>, S^y|down> = -i/2 |up>: flipping
+ *        bit b contributes the factor i (2 b - 1) / 2 = i sigma_b)
+ * The sums are real (the i -> i xor m terms pair up as complex conjugates); the real part is accumulated. */
+double tso_correlate(const double *psi, int N, int alpha, int j, int k)
+{
+    const int64_t dim = (int64_t)1 << N;
+    const int64_t bj = (int64_t)1 << j, bk = (int64_t)1 << k, m = bj | bk;
+    double sum = 0.0, comp = 0.0;
+    for (int64_t i = 0; i < dim; ++i) {
+        const double sj = (i & bj) ? 0.5 : -0.5, sk = (i & bk) ? 0.5 : -0.5;
+        const double r0 = psi[2 * i], i0 = psi[2 * i + 1];
+        double term;
+        if (alpha == TSO_Z) {
+            term = sj * sk * (r0 * r0 + i0 * i0);
+        } else {
+            const double r1 = psi[2 * (i ^ m)], i1 = psi[2 * (i ^ m) + 1];
+            const double re = r1 * r0 + i1 * i0;                 /* Re( conj(c_{i xor m}) c_i ) */
+            term = (alpha == TSO_X) ? 0.25 * re : -sj * sk * re;
+        }
+        double y = term - comp;
+        double t = sum + y;
+        comp = (t - sum) - y;
+        sum = t;
+    }
+    return sum;
+}
+
+/* Total magnetisation sum_j <S^z_j> ("the spurious total magnetization observed in polarization-conserving
+ * Hamiltonians"). */
+double tso_total_sz(const double *psi, int N)
+{
+    double s = 0.0;
+    for (int j = 0; j < N; ++j) s += tso_expect(psi, N, TSO_Z, j);
+    return s;
+}
+
+/* <psi|H|psi> for the Hamiltonian of eq. 1, term by term from the definition:
+ *   sum_a [ sum_j h^a_j <S^a_j>  +  sum_{j != k} J^a_{jk} <S^a_j S^a_k> ]        (diagonal of J ignored, A1). */
+double tso_energy_expect(const double *psi, int N, const double *h, const double *J)
+{
+    double E = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        for (int j = 0; j < N; ++j) {
+            const double hj = h[(size_t)a * N + j];
+            if (hj != 0.0) E += hj * tso_expect(psi, N, a, j);
+        }
+        for (int j = 0; j < N; ++j)
+            for (int k = 0; k < N; ++k) {
+                if (j == k) continue;
+                const double Jjk = J[((size_t)a * N + j) * N + k];
+                if (Jjk != 0.0) E += Jjk * tso_correlate(psi, N, a, j, k);
+            }
+    }
+    return E;
+}
+
+/* The "one spin up, the rest in high-temperature equilibrium" state of eq. A.1:
+ *   |Psi_0> = |up>_u (x) sum_{j < 2^(N-1)} 2^{-(N-1)/2} exp(i phi_j) |beta_j>,   phi_j = random phase.
+ * |beta_j> runs over the Ising states of the other N-1 spins: j is the amplitude index with bit u removed.
+ * The paper does not say how the phases are drawn; here phi_j = 2 pi u_j with u_j in [0, 1) from a COUNTER-BASED
+ * generator, so that the oracle and the CUDA path can each produce phase j without sharing code or state:
+ *   u_j = (splitmix64(seed + (j + 1) * 0x9E3779B97F4A7C15) >> 11) * 2^-53
+ * where splitmix64 is the finalizer of Steele, Lea & Flood's SplitMix generator (i.e. u_j is the (j+1)-th output of
+ * SplitMix64 seeded with `seed`; pinned by its published first outputs for seed 0 in the tests). */
+static uint64_t splitmix64_mix(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * UINT64_C(0xBF58476D1CE4E5B9);
+    z = (z ^ (z >> 27)) * UINT64_C(0x94D049BB133111EB);
+    return z ^ (z >> 31);
+}
+
+uint64_t tso_splitmix64(uint64_t seed, uint64_t j)
+{
+    return splitmix64_mix(seed + (j + 1) * UINT64_C(0x9E3779B97F4A7C15));
+}
+
+void tso_random_phase_state(double *psi, int N, int up_spin, uint64_t seed)
+{
+    const int64_t dim = (int64_t)1 << N;
+    const int64_t ub = (int64_t)1 << up_spin;
+    const double amp = 1.0 / sqrt(ldexp(1.0, N - 1));
+    for (int64_t k = 0; k < dim; ++k) {
+        if (!(k & ub)) { psi[2 * k] = 0.0; psi[2 * k + 1] = 0.0; continue; }
+        const uint64_t j = (uint64_t)(((k >> (up_spin + 1)) << up_spin) | (k & (ub - 1)));   /* k with bit u removed */
+        const double u = (double)(tso_splitmix64(seed, j) >> 11) * ldexp(1.0, -53);
+        const double phi = 2.0 * 3.14159265358979323846 * u;    /* 2 pi u (-std=c99 has no M_PI) */
+        psi[2 * k] = amp * cos(phi);
+        psi[2 * k + 1] = amp * sin(phi);
+    }
+}

@@ -52,6 +52,16 @@ def _load():
     lib.tso_norm2.argtypes = [_dp, ctypes.c_int]
     lib.tso_overlap.restype = None
     lib.tso_overlap.argtypes = [_dp, _dp, ctypes.c_int, _dp]
+    lib.tso_correlate.restype = ctypes.c_double
+    lib.tso_correlate.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+    lib.tso_total_sz.restype = ctypes.c_double
+    lib.tso_total_sz.argtypes = [_dp, ctypes.c_int]
+    lib.tso_energy_expect.restype = ctypes.c_double
+    lib.tso_energy_expect.argtypes = [_dp, ctypes.c_int, _dp, _dp]
+    lib.tso_splitmix64.restype = ctypes.c_uint64
+    lib.tso_splitmix64.argtypes = [ctypes.c_uint64, ctypes.c_uint64]
+    lib.tso_random_phase_state.restype = None
+    lib.tso_random_phase_state.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_uint64]
     _lib = lib
     return lib
 
@@ -143,3 +153,31 @@ def overlap(phi, psi, N) -> complex:
     out = np.zeros(2)
     _load().tso_overlap(_psi_ptr(phi, N), _psi_ptr(psi, N), N, out.ctypes.data_as(_dp))
     return complex(out[0], out[1])
+
+
+def correlate(psi, N, alpha, j, k) -> float:
+    """<psi| S^alpha_j S^alpha_k |psi>, j != k."""
+    assert j != k
+    return float(_load().tso_correlate(_psi_ptr(psi, N), N, alpha, j, k))
+
+
+def total_sz(psi, N) -> float:
+    return float(_load().tso_total_sz(_psi_ptr(psi, N), N))
+
+
+def energy_expect(psi, N, h, J) -> float:
+    """<psi|H|psi> for eq. 1, from one- and two-site expectation values."""
+    h = _f64(h, (3, N))
+    J = _f64(J, (3, N, N))
+    return float(_load().tso_energy_expect(_psi_ptr(psi, N), N, h.ctypes.data_as(_dp), J.ctypes.data_as(_dp)))
+
+
+def splitmix64(seed, j) -> int:
+    return int(_load().tso_splitmix64(ctypes.c_uint64(seed), ctypes.c_uint64(j)))
+
+
+def random_phase_state(N, up_spin, seed) -> np.ndarray:
+    """Eq. A.1: spin `up_spin` up, the other N-1 spins in an equal-weight random-phase superposition."""
+    psi = np.empty(1 << N, dtype=np.complex128)
+    _load().tso_random_phase_state(_psi_ptr(psi, N), N, up_spin, ctypes.c_uint64(seed))
+    return psi
