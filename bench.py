@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- Trotter-Suzuki steps/s at N = 30 on B200 (BASELINE.json metric), with roofline and CPU baseline.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--N 30] [--no-e2e] [--no-cpu]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--N 30] [--config 1|2|3|4|5]
+                    [--repeats 5] [--no-e2e] [--no-cpu] [--cpu-full]
 
 A "step" is one 4th-order Trotter-Suzuki step U_4(tau) (20 global rotations + 20 merged diagonals) of
 the whole 2^N complex128 state of the metric workload (workloads.config("M"): 5x6 open XYZ lattice, N = 30, 16 GiB).
@@ -105,46 +106,95 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------------- CPU oracle legs
-def oracle_sample(N_metric: int, w_metric: W.Workload):
-    """One 4th-order step of the SAME lattice recipe at a size the oracle finishes in ~10-30 s, scaled to the metric
-    size by the oracle's own cost model (work per step ~ N 2^N)."""
+def cpu_info():
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except Exception:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count(), "OMP_NUM_THREADS": os.environ.get("OMP_NUM_THREADS", "unset")}
+
+
+def oracle_steps_per_s(Ns: int, n_steps: int):
+    """The oracle as it stands (plain C + OpenMP on all host cores) on the open-lattice XYZ recipe at size Ns:
+    n_steps single 4th-order steps, each timed; returns (median steps/s, [seconds])."""
     from oracle import ts_oracle as O
-    Ns = min(N_metric, 24)
-    ws = w_metric if Ns == N_metric else W.grid_like(Ns, seed=8, tau=w_metric.tau, n_steps=1, state_seed=9, cols=6)
+    ws = W.grid_like(Ns, seed=8, tau=0.01, n_steps=1, state_seed=9, cols=6 if Ns >= 24 else None)
     psi = ws.state()
     O.evolve(psi, Ns, ws.h, ws.J, ws.tau, 0, 4, True)          # loads the library
-    t = time.perf_counter()
-    O.evolve(psi, Ns, ws.h, ws.J, ws.tau, 1, 4, True)
-    dt = time.perf_counter() - t
-    scale = (2.0 ** (Ns - N_metric)) * (Ns / N_metric)
-    return {"steps_per_s_sample": 1.0 / dt, "value": scale / dt, "N_sample": Ns, "seconds": dt,
-            "cores": O.num_threads(),
-            "sample": f"1 U4 step of the same open-lattice XYZ recipe at N={Ns} (oracle as it stands, OpenMP), "
-                      f"scaled by 2^({Ns}-{N_metric})*{Ns}/{N_metric} to N={N_metric}"}
+    secs = []
+    for _ in range(n_steps):
+        t = time.perf_counter()
+        O.evolve(psi, Ns, ws.h, ws.J, ws.tau, 1, 4, True)
+        secs.append(time.perf_counter() - t)
+    return 1.0 / float(np.median(secs)), secs
+
+
+def oracle_baseline(N_metric: int, full: bool):
+    """BASELINE.md's CPU-baseline plan: measured at N = 22 (3 steps, median) and N = 27 (1 step by default so that the
+    run stays within minutes; 3 steps, median, with --cpu-full), and the metric size extrapolated from the largest
+    measured size by the oracle's own cost model (work per step ~ N 2^N), labelled as such."""
+    from oracle import ts_oracle as O
+    sizes = [(min(22, N_metric), 3)]
+    if N_metric > 22:
+        sizes.append((min(27, N_metric), 3 if full else 1))
+    measured = {}
+    for Ns, k in sizes:
+        v, secs = oracle_steps_per_s(Ns, k)
+        measured[f"N={Ns}"] = {"steps_per_s": v, "seconds_per_step": [round(x, 3) for x in secs], "steps_timed": k}
+    Nl = sizes[-1][0]
+    scale = (2.0 ** (Nl - N_metric)) * (Nl / N_metric)
+    value = measured[f"N={Nl}"]["steps_per_s"] * scale
+    info = cpu_info()
+    out = {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "measured": measured,
+           "extrapolated": Nl != N_metric,
+           "sample": (f"oracle as it stands (plain C, OpenMP, {O.num_threads()} threads) on the same open-lattice XYZ recipe: "
+                      + ", ".join(f"{k}: {v['steps_timed']} step(s), median" for k, v in measured.items())
+                      + (f"; N={N_metric} value EXTRAPOLATED from N={Nl} by 2^({Nl}-{N_metric})*{Nl}/{N_metric}"
+                         if Nl != N_metric else "")),
+           **info}
+    return out
 
 
 def run_reference(args):
+    """The reference arm of this tier IS the oracle (there is no reference program): K timed single steps of the oracle, as
+    it stands, on a bounded sample of the workload -- the same lattice recipe at N = 24, ~5 s per step on 16 cores, so
+    that `--steps 20 --warmup 5` ends within a few minutes -- scaled to the metric size by its cost model (~ N 2^N)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    from oracle import ts_oracle as O
     w = workload_for(args.N)
+    Ns = min(24, args.N)
+    ws = w if Ns == args.N else W.grid_like(Ns, seed=8, tau=w.tau, n_steps=1, state_seed=9, cols=6)
+    psi = ws.state()
+    O.evolve(psi, Ns, ws.h, ws.J, ws.tau, 0, 4, True)          # loads the library
     times = []
-    info = None
     for i in range(args.warmup + args.steps):
-        info = oracle_sample(args.N, w)
+        t = time.perf_counter()
+        O.evolve(psi, Ns, ws.h, ws.J, ws.tau, 1, 4, True)
+        dt = time.perf_counter() - t
         if i >= args.warmup:
-            times.append(info["seconds"])
-        if sum(times) > 150:           # keep the whole run within a few minutes
+            times.append(dt)
+        if sum(times) > 150:                   # keep the whole run within a few minutes
             break
+    if not times:
+        times = [dt]
     n_done = len(times)
-    scale = (2.0 ** (info["N_sample"] - args.N)) * (info["N_sample"] / args.N)
+    scale = (2.0 ** (Ns - args.N)) * (Ns / args.N)
     value = scale * n_done / sum(times)
+    sample = (f"{n_done} timed oracle step(s) at N={Ns} (open-lattice XYZ recipe, plain C + OpenMP, {O.num_threads()} threads)"
+              + (f", EXTRAPOLATED to N={args.N} by 2^({Ns}-{args.N})*{Ns}/{args.N}" if Ns != args.N else ""))
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
            "steps": n_done, "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
            "config": {"workload": w.name, "N": args.N, "order": 4, "tau": w.tau},
-           "cpu_baseline": {"value": value, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
-                            "sample": info["sample"]},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample,
+                            "extrapolated": Ns != args.N, **cpu_info()},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out))
 
@@ -155,6 +205,37 @@ def fill_pinned_state(w: W.Workload, host):
     hv = host.numpy()
     for first, chunk in w.state_chunks(chunk_log2=22):
         hv[first:first + chunk.size] = chunk
+
+
+def kernel_sources_hash() -> str:
+    """SHA-256 over the CUDA sources: an ncu capture under profiles/ is only quoted for the build it was taken from."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1305_0036_b200", "csrc")
+    hsh = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            with open(os.path.join(d, name), "rb") as f:
+                hsh.update(name.encode() + b"\0" + f.read())
+    return hsh.hexdigest()[:16]
+
+
+def recorded_traffic(kernel_class: str, N: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel_class` from the newest committed ncu capture
+    (profiles/r02_traffic.csv: columns class,N,dram_read_bytes,dram_write_bytes,sources_hash,commit), or None when that
+    capture belongs to other kernel sources than the ones being timed."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as f:
+            rows = [ln.strip().split(",") for ln in f if ln.strip() and not ln.startswith("#")]
+    except Exception:
+        return None
+    cur = kernel_sources_hash()
+    for r in rows[1:]:
+        if len(r) >= 6 and r[0] == kernel_class and int(r[1]) == N:
+            if r[4] != cur:
+                return None
+            return {"bytes": float(r[2]) + float(r[3]), "read": float(r[2]), "write": float(r[3]), "commit": r[5],
+                    "sources_hash": r[4]}
+    return None
 
 
 def run_ours(args):
@@ -172,14 +253,23 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    N = args.N
-    w = workload_for(N, args.workload)
+    if args.config:
+        w = W.config(int(args.config))     # BASELINE configs 1-5 (parity-test cases; timed here on request only)
+        N = w.N
+    else:
+        N = args.N
+        w = workload_for(N, args.workload)
     if world > 1:                      # independent ensemble members: same Hamiltonian, different random state
         w.state_seed = R.replica_state_seed(w.state_seed, rank)
     dim = 1 << N
     ts = B.TrotterSuzuki(N, w.h, w.J, device=str(dev))
     if args.plan:
         ts.set_plan(*[int(x) for x in args.plan.split(",")])
+    if args.groups:
+        ts.set_plan_groups([int(x) for x in args.groups.split(",")])
+    for kv in args.opt:
+        k, v = kv.split("=")
+        ts.set_option(getattr(B, "OPT_" + k.upper()), int(v))
     host = torch.empty(dim, dtype=torch.complex128, pin_memory=True)
     fill_pinned_state(w, host)
     ts.set_state(host)
@@ -190,29 +280,38 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing
+    # ---- device-resident timing: `repeats` regions of exactly K steps each, every region bracketed by a barrier and a
+    # device synchronisation on both sides and timed with CUDA events on the stream the kernels run on; the value is
+    # taken from the MEDIAN region (max over ranks of each region).  The state (16 * 2^N bytes) is larger than L2 for
+    # N >= 24; for smaller N the L2 is flushed before every region.
     ts.set_profiling(os.environ.get('TS_BENCH_NOPROF', '0') != '1')
     for _ in range(max(args.warmup, 3)):
         ts.evolve(w.tau, 1, 4)
     barrier()
-    ts.reset_profile()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if 16 * dim < (256 << 20) else None
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
+    region_ms, prof = [], None
     t0 = time.time()
-    e0.record()
-    ts.evolve(w.tau, args.steps, 4)
-    e1.record()
-    barrier()
+    for rep in range(max(args.repeats, 1)):
+        if flush is not None:
+            flush.fill_(rep)
+        if rep == max(args.repeats, 1) - 1:
+            ts.reset_profile()             # per-kernel-class event times of the last region
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        ts.evolve(w.tau, args.steps, 4)
+        e1.record()
+        barrier()
+        region_ms.append(R.max_over_ranks(e0.elapsed_time(e1), dev))
     t1 = time.time()
-    ms = e0.elapsed_time(e1)
     prof = ts.get_profile()
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     norm2 = ts.norm2()
-    ms = R.max_over_ranks(ms, dev)
+    ms = float(np.median(region_ms))
     steps_per_s = R.whole_job_steps_per_s(args.steps, world, ms)
 
     # ---- end to end through the C ABI with host buffers: H2D of the state + 1 step + D2H of <S^z_j>
@@ -238,56 +337,65 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (fused tile pass): algorithmic bytes = read + write of the state once
+    # ---- roofline.  Unit = one amplitude; algorithmic bytes = 32 B per amplitude per HBM ROUND TRIP of
+    # the state (16 B read + 16 B written), and every tile launch -- a fused pass, a single pass, or an L2-blocked triple
+    # launch, which performs three tile passes on L2-resident chunks -- makes exactly one round trip of all 2^N
+    # amplitudes.  So achieved = 32 * 2^N / launch time is what the HBM had to deliver, NOT a credit for passes: the
+    # three passes' worth (SURVEY 8 d's contract figure) is reported separately as `credited_*`.
     peak, peak_src = measured_peak()
-    # Algorithmic bytes: 32 B per amplitude per tile pass (read + write of the state once).  A
-    # "tile_chunk3" launch does the work of THREE tile passes (high . fused low . high) and is credited with three
-    # passes' bytes, SURVEY 8(d)'s per-pass figure; because it keeps each 32 MiB chunk in L2 between them it needs only
-    # ONE HBM round trip ("hbm_round_trip_bytes_per_launch"): fewer bytes moved than credited is the point of it.
-    pass_bytes = 32.0 * dim
-    passes_per_launch = {"tile_fused": 1, "tile_single": 1, "tile_chunk3": 3, "naive_rot": 1, "naive_diag": 1}
-    dom = max(passes_per_launch, key=lambda k: prof[k]["ms"])
-    alg_bytes = pass_bytes * passes_per_launch[dom]
+    rt_bytes = 32.0 * dim
+    tile_classes = ("tile_fused", "tile_single", "tile_chunk3")
+    timed = {k: prof[k] for k in tile_classes + ("naive_rot", "naive_diag", "small") if prof[k]["launches"]}
+    dom = max(timed, key=lambda k: timed[k]["ms"]) if timed else "tile_fused"
     dms = prof[dom]["ms"] / max(prof[dom]["launches"], 1)
-    achieved = alg_bytes / (dms * 1e-3) / 1e9 if dms > 0 else 0.0
-    kern_ms = {k: v for k, v in prof.items() if v["launches"]}
+    achieved = rt_bytes / (dms * 1e-3) / 1e9 if dms > 0 else 0.0
+    kern = {}
+    for k, v in prof.items():
+        if not v["launches"]:
+            continue
+        kern[k] = dict(v)
+        if k in tile_classes and v["ms"] > 0:
+            kern[k]["avg_ms"] = v["ms"] / v["launches"]
+            kern[k]["hbm_gbs"] = v["launches"] * rt_bytes / (v["ms"] * 1e-3) / 1e9
+            kern[k]["credited_gbs"] = v["state_passes"] * rt_bytes / (v["ms"] * 1e-3) / 1e9
     launches = sum(v["launches"] for v in prof.values())
-    round_trips = prof["tile_fused"]["launches"] + prof["tile_single"]["launches"] + prof["tile_chunk3"]["launches"]
-    tile_passes = prof["tile_fused"]["launches"] + prof["tile_single"]["launches"] + 3 * prof["tile_chunk3"]["launches"]
     step_ms = ms / args.steps
-    traffic = None                    # dram__bytes_read + write of the dominant kernel from the committed ncu capture (N = 30)
-    try:                              # (values and the command that produced them: profiles/r01b_pipeline_and_l2_blocking.md)
-        with open(os.path.join(ROOT, "profiles", "r01b_traffic.csv")) as f:
-            for line in f.read().splitlines()[1:]:
-                k, rd, wr = line.split(",")
-                if N == 30 and k == dom:
-                    traffic = float(rd) + float(wr)
-    except Exception:
-        traffic = None
+    round_trips = sum(prof[k]["launches"] for k in tile_classes) / args.steps
+    tile_passes = sum(prof[k]["state_passes"] for k in tile_classes) / args.steps
+    tr = recorded_traffic(dom, N)
+    hbm_resident = 16 * dim > (126 << 20)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic,
-                "alg_bytes_per_launch": alg_bytes, "tile_passes_per_launch": passes_per_launch[dom],
-                "hbm_round_trip_bytes_per_launch": pass_bytes, "avg_launch_ms": dms,
-                "step_gbs_over_tile_passes": tile_passes * pass_bytes / (ms * 1e-3) / 1e9,
-                "step_gbs_over_hbm_round_trips": round_trips * pass_bytes / (ms * 1e-3) / 1e9,
-                "contract_model_frac_of_8TBs": (N_SWEEPS_PER_STEP * (1 + -(-(N - 13) // 10) if N > 13 else 1)
-                                                * pass_bytes / 8e12) / (step_ms * 1e-3)}
+                "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": tr["bytes"] if tr else None, "traffic_capture": tr,
+                "frac_dram_actual": (tr["bytes"] / (dms * 1e-3) / 1e9 / peak) if (tr and dms > 0) else None,
+                "alg_bytes_per_launch": rt_bytes, "avg_launch_ms": dms,
+                "credited_tile_passes_per_launch": prof[dom]["state_passes"] / max(prof[dom]["launches"], 1),
+                "credited_gbs": kern.get(dom, {}).get("credited_gbs"),
+                "step": {"hbm_round_trips": round_trips, "tile_passes": tile_passes,
+                         "bytes_moved": round_trips * rt_bytes, "gbs": round_trips * rt_bytes / (step_ms * 1e-3) / 1e9,
+                         "frac_of_peak": round_trips * rt_bytes / (step_ms * 1e-3) / 1e9 / peak,
+                         "floor_round_trips": N_SWEEPS_PER_STEP,
+                         "contract_model_frac_of_8TBs": (N_SWEEPS_PER_STEP * (1 + -(-(N - 13) // 10) if N > 13 else 1)
+                                                         * rt_bytes / 8e12) / (step_ms * 1e-3)},
+                "note": None if hbm_resident else "state fits in L2: absolute steps/s is the figure, not an HBM fraction"}
     cpu = None
     if not args.no_cpu:
-        s = oracle_sample(N, workload_for(N))      # (always the lattice recipe: the oracle's cost does not depend on it)
-        cpu = {"value": s["value"], "unit": UNIT, "cores": s["cores"], "kind": "oracle", "sample": s["sample"],
-               "sample_steps_per_s": s["steps_per_s_sample"]}
+        cpu = oracle_baseline(N, args.cpu_full)     # (the lattice recipe: the oracle's cost does not depend on the Hamiltonian)
 
     out = {"metric": METRIC, "value": steps_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
            "config": {"workload": w.name, "N": N, "order": 4, "tau": w.tau, "state_bytes": 16 * dim,
-                      "plan": ts.describe_plan(), "l2": "state (16*2^N B) is larger than L2; no flush needed",
+                      "plan": ts.describe_plan(),
+                      "l2": ("state (16*2^N B) is larger than L2; no flush needed" if flush is None
+                             else "L2 flushed (256 MiB write) before every timed region"),
                       "parallelism": f"replicas x{world}" if world > 1 else "1 GPU"},
+           "timing": {"regions": len(region_ms), "region_ms": [round(x, 3) for x in region_ms], "value_from": "median region",
+                      "steps_per_region": args.steps},
            "spin_amplitude_updates_per_sec": steps_per_s * N_SWEEPS_PER_STEP * N * dim,
            "amplitude_steps_per_sec": steps_per_s * dim,
-           "norm2_after": norm2,
-           "gpu_launches": launches, "kernels": kern_ms, "clocks": clocks, "roofline": roofline,
+           "norm2_after": norm2, "library": B.version(), "kernel_sources_hash": kernel_sources_hash(),
+           "gpu_launches": launches, "kernels": kern, "clocks": clocks, "roofline": roofline,
            "cpu_baseline": cpu, "e2e": e2e}
     print(json.dumps(out))
     if world > 1:
@@ -304,6 +412,11 @@ def main():
     ap.add_argument("--workload", default="grid", choices=["grid", "chain", "dipolar"],
                     help="Hamiltonian family (north_star: chains, lattices, all-to-all); the metric line is the default grid")
     ap.add_argument("--plan", default="", help="mode,run_bits,max_group_bits (ts_set_plan)")
+    ap.add_argument("--groups", default="", help="bits of the high groups, bottom to top (ts_set_plan_groups), e.g. 9,9")
+    ap.add_argument("--opt", action="append", default=[], help="KEY=VALUE for ts_set_option, e.g. kernel=0, chunk=0")
+    ap.add_argument("--config", default="", help="time BASELINE config 1..5 instead of the metric workload")
+    ap.add_argument("--repeats", type=int, default=5, help="timed regions of K steps each; the value is their median")
+    ap.add_argument("--cpu-full", action="store_true", help="oracle: 3 steps (median) at N = 27 instead of 1")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

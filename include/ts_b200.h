@@ -49,7 +49,8 @@ enum { TS_KC_TILE_FUSED = 0,   /* tile pass: sweep . diagonal . sweep in one HBM
        TS_KC_REDUCE = 4,       /* observable / norm reductions */
        TS_KC_SETUP = 5,        /* phase-table construction, state initialisation */
        TS_KC_TILE_CHUNK = 6,   /* three tile passes (high . fused low . high) in one L2-blocked launch: 1 HBM round trip */
-       TS_KC_COUNT = 7 };
+       TS_KC_SMALL = 7,        /* N <= 12: a whole ts_evolve call in one single-CTA launch */
+       TS_KC_COUNT = 8 };
 
 /* Problem statement (eq. 1).  N in [1, 33].  h: [3][N], J: [3][N][N]; both are COPIED.
  * Errors: TS_ERR_ARG (null pointer, N out of range, non-finite h or J), TS_ERR_CUDA (no device), TS_ERR_NOMEM. */
@@ -107,13 +108,71 @@ int ts_norm2(ts_ctx* ctx, double* out);
 /* out[0], out[1] = Re, Im of <phi|psi> where phi is a DEVICE buffer of 2^N complex128 (eq. 11). */
 int ts_overlap(ts_ctx* ctx, const void* dev_phi, double* out);
 
-/* Execution plan.  mode: TS_PLAN_AUTO (tiled when N >= 12, else naive), TS_PLAN_NAIVE (one launch per spin rotation
+/* out[0] = <psi| S^alpha_j S^alpha_k |psi>, j != k (two-site correlator: the "non-local physical magnitudes" of P:203;
+ * formulas in csrc/ts_reduce.cu, reading A15).  One read-only pass.  Synchronises.  Errors: TS_ERR_ARG (j = k, range). */
+int ts_correlate(ts_ctx* ctx, int alpha, int j, int k, double* out);
+
+/* out[0] = sum_j <psi|S^z_j|psi>, the total magnetisation (conserved by polarisation-conserving Hamiltonians;
+ * its spurious drift is the paper's second accuracy test).  One pass.  Synchronises. */
+int ts_total_sz(ts_ctx* ctx, double* out);
+
+/* out[0] = <psi|H|psi> for the Hamiltonian of eq. 1.  <H_z> is a weighted sum of |c_k|^2; <H_x> and <H_y> are
+ * the same sums in the frames rotated by Y^dag and X^dag (eq. 7, 10), so the call applies four global rotations to the
+ * state and undoes them exactly up to round-off: the state returns changed by <= ~1e-15 relative.  The energies are
+ * evaluated from the O(N^2) definition -- an observable, not part of the time step.  Synchronises. */
+int ts_energy(ts_ctx* ctx, double* out);
+
+/* State := the "one spin up, the rest at infinite temperature" pure state of eq. A.1:
+ *   |up>_u (x) sum_j 2^{-(N-1)/2} exp(i phi_j) |beta_j>,  phi_j = 2 pi u_j,
+ * u_j = (j+1)-th output of SplitMix64 seeded with `seed`, top 53 bits (a counter-based stream, so ensemble members
+ * are reproducible from (seed) alone; the oracle restates the same generator).  Allocates like ts_set_state. */
+int ts_set_random_phase_state(ts_ctx* ctx, int up_spin, uint64_t seed);
+
+/* Loschmidt echo with Sigma = 0 (eq. 11): keeps a device copy psi_0 of the current state, applies
+ * [U_order(tau)]^n then [U_order(-tau)]^n, and returns out[0] = M_LE = |<psi_0|psi>|^2, out[1], out[2] = Re, Im of the
+ * overlap.  For a perfectly accurate computation M_LE = 1: the deviation measures floating-point round-off only
+ * (P:215).  Needs 16 * 2^N bytes of scratch.  Synchronises.  Errors: as ts_evolve, TS_ERR_NOMEM. */
+int ts_loschmidt_echo(ts_ctx* ctx, double tau, int64_t n_steps, int order, double* out /*[3]*/);
+
+/* Execution plan.  mode: TS_PLAN_AUTO (N <= 12: one single-CTA launch per ts_evolve; N >= 13: tiled), TS_PLAN_NAIVE (one launch per spin rotation
  * and per diagonal: the paper's basic scheme, kept as bring-up path and A/B baseline), TS_PLAN_TILED.
  * run_bits: number s of lowest index bits kept inside every high-bit tile (runs of 2^s * 16 bytes),
  * 0 = default (3).  max_group_bits: upper bound on butterflied bits per high-bit pass, 0 = as many as fit
  * (12 - s); smaller values force more passes (used by tests to exercise multi-group plans at small N).
  * Errors: TS_ERR_ARG when the combination cannot be planned for this N. */
 int ts_set_plan(ts_ctx* ctx, int mode, int run_bits, int max_group_bits);
+
+/* Explicit plan: the number of index bits of every high group, bottom to top (group k butterflies the high_bits[k]
+ * spins above group k-1; group A = spins 0..11 is implied).  sum(high_bits) must be N - 12, each entry in [1, 11];
+ * entries <= 9 (runs of >= 128 bytes) run on the pipelined kernels.  This is what the tuner
+ * (paper_1305_0036_b200/tuner.py; "a brute force search for the fastest series of rotations ... stored in a
+ * file") searches over and what a stored plan file sets.  N >= 12 only.  Errors: TS_ERR_ARG. */
+int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
+
+/* Execution options (all have defaults; the tuner and the A/B benchmarks set them).
+ *   TS_OPT_KERNEL          1 (default): warp-specialised TMA kernels; 0: one CTA per tile, register loads
+ *   TS_OPT_CHUNK           1 (default): [high . fused low . high] as one L2-blocked launch where the plan allows; 0: off
+ *   TS_OPT_CHUNK_MAX_LOG2  largest chunk of the L2-blocked launch, log2 amplitudes (default 21 = 32 MiB), 13..26
+ *   TS_OPT_L2_PROMOTION    tensor-map L2 promotion of the high groups: 0 none (default), 1: 128 B, 2: 256 B
+ *   TS_OPT_SMALL           1 (default): under TS_PLAN_AUTO, N <= 12 runs a whole ts_evolve call as one single-CTA launch
+ *                          (state in shared memory; small systems are latency-bound); 0: tiled / naive plans
+ *   TS_OPT_DIAG_SOURCE     TS_PLAN_NAIVE only: 0 (default) each diagonal evaluates the O(N^2) energy per amplitude;
+ *                          1: the paper's pre-computed variant: three 2^N-element energy vectors (+24 bytes per
+ *                          amplitude), built on first use -- the A/B experiment of DESIGN.md 7.5
+ *   TS_OPT_MAX_CTAS        upper bound on the grid of the persistent tile kernels (0, default: one CTA per SM); small values
+ *                          make every CTA walk many tiles -- used by the tests to exercise buffer reuse at small N
+ * Errors: TS_ERR_ARG (unknown key, value out of range). */
+enum { TS_OPT_KERNEL = 0, TS_OPT_CHUNK = 1, TS_OPT_CHUNK_MAX_LOG2 = 2, TS_OPT_L2_PROMOTION = 3, TS_OPT_SMALL = 4,
+       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6 };
+int ts_set_option(ts_ctx* ctx, int key, int value);
+int ts_get_option(ts_ctx* ctx, int key, int* value);
+
+/* Apply the line for this context's N of a plan file written by the tuner ("stored in a file"):
+ *     N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 l2_promotion=0
+ * (text; '#' starts a comment line; keys other than N may be omitted).  No line for this N: TS_OK, nothing changes.
+ * ts_create applies the file named by the environment variable TS_PLAN_FILE, if set, the same way.
+ * Errors: TS_ERR_ARG (file cannot be opened, or the line does not describe a valid plan for N). */
+int ts_load_plan_file(ts_ctx* ctx, const char* path);
 
 /* Human-readable description of the current plan (groups, passes per sweep) into buf (NUL-terminated). */
 int ts_describe_plan(ts_ctx* ctx, char* buf, int buflen);
@@ -124,6 +183,9 @@ int ts_describe_plan(ts_ctx* ctx, char* buf, int buflen);
 int ts_set_profiling(ts_ctx* ctx, int enable);
 int ts_get_profile(ts_ctx* ctx, int64_t* launches /*[TS_KC_COUNT]*/, double* ms /*[TS_KC_COUNT]*/);
 int ts_reset_profile(ts_ctx* ctx);
+/* state_passes[c]: tile passes over the WHOLE state performed by the launches of class c since the last reset (1 per tile
+ * pass launch, 3 per L2-blocked triple launch, 0 for the other classes): what bench.py turns into bytes. */
+int ts_get_profile_passes(ts_ctx* ctx, double* state_passes /*[TS_KC_COUNT]*/);
 
 /* Static string for a status code. */
 const char* ts_strerror(int status);

@@ -18,13 +18,16 @@ TS_OK, TS_ERR_ARG, TS_ERR_NOMEM, TS_ERR_CUDA, TS_ERR_NOSTATE = 0, -1, -2, -3, -4
 X, Y, Z = 0, 1, 2
 HOST, DEVICE = 0, 1
 PLAN_AUTO, PLAN_NAIVE, PLAN_TILED = 0, 1, 2
-KC_NAMES = ("tile_fused", "tile_single", "naive_rot", "naive_diag", "reduce", "setup", "tile_chunk3")
+OPT_KERNEL, OPT_CHUNK, OPT_CHUNK_MAX_LOG2, OPT_L2_PROMOTION, OPT_SMALL, OPT_DIAG_SOURCE, OPT_MAX_CTAS = 0, 1, 2, 3, 4, 5, 6
+KC_NAMES = ("tile_fused", "tile_single", "naive_rot", "naive_diag", "reduce", "setup", "tile_chunk3", "small")
 KC_COUNT = len(KC_NAMES)
 
 # every symbol include/ts_b200.h declares (tests check that the library exports all of them)
 SYMBOLS = ("ts_create", "ts_destroy", "ts_set_stream", "ts_bind_state", "ts_set_state", "ts_set_basis_state",
            "ts_set_state_range", "ts_get_state", "ts_evolve", "ts_evolve_observe", "ts_expect", "ts_expect_all", "ts_norm2", "ts_overlap", "ts_set_plan",
-           "ts_describe_plan", "ts_set_profiling", "ts_get_profile", "ts_reset_profile", "ts_strerror", "ts_version")
+           "ts_describe_plan", "ts_set_profiling", "ts_get_profile", "ts_reset_profile", "ts_strerror", "ts_version",
+           "ts_set_plan_groups", "ts_set_option", "ts_get_option", "ts_get_profile_passes", "ts_correlate", "ts_total_sz",
+           "ts_energy", "ts_set_random_phase_state", "ts_loschmidt_echo", "ts_load_plan_file")
 
 _lib = None
 _vp, _dp, _i64p = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)
@@ -63,6 +66,16 @@ def load() -> ctypes.CDLL:
         "ts_overlap": (I, [_vp, _vp, _dp]),
         "ts_set_plan": (I, [_vp, I, I, I]),
         "ts_describe_plan": (I, [_vp, ctypes.c_char_p, I]),
+        "ts_set_plan_groups": (I, [_vp, I, ctypes.POINTER(I)]),
+        "ts_set_option": (I, [_vp, I, I]),
+        "ts_load_plan_file": (I, [_vp, ctypes.c_char_p]),
+        "ts_get_option": (I, [_vp, I, ctypes.POINTER(I)]),
+        "ts_get_profile_passes": (I, [_vp, _dp]),
+        "ts_correlate": (I, [_vp, I, I, I, _dp]),
+        "ts_total_sz": (I, [_vp, _dp]),
+        "ts_energy": (I, [_vp, _dp]),
+        "ts_set_random_phase_state": (I, [_vp, I, U64]),
+        "ts_loschmidt_echo": (I, [_vp, D, I64, I, _dp]),
         "ts_set_profiling": (I, [_vp, I]),
         "ts_get_profile": (I, [_vp, _i64p, _dp]),
         "ts_reset_profile": (I, [_vp]),
@@ -132,6 +145,23 @@ class TrotterSuzuki:
 
     def set_plan(self, mode: int = PLAN_AUTO, run_bits: int = 0, max_group_bits: int = 0):
         _check(self._lib.ts_set_plan(self._ctx, mode, run_bits, max_group_bits), "ts_set_plan")
+
+    def set_plan_groups(self, high_bits):
+        """Explicit bits of every high group, bottom to top (sum = N - 12)."""
+        arr = (ctypes.c_int * len(high_bits))(*[int(b) for b in high_bits])
+        _check(self._lib.ts_set_plan_groups(self._ctx, len(high_bits), arr), "ts_set_plan_groups")
+
+    def load_plan_file(self, path: str):
+        """Apply the tuned plan stored for this N in a plan file (paper_1305_0036_b200/tuner.py writes them)."""
+        _check(self._lib.ts_load_plan_file(self._ctx, str(path).encode()), "ts_load_plan_file")
+
+    def set_option(self, key: int, value: int):
+        _check(self._lib.ts_set_option(self._ctx, int(key), int(value)), "ts_set_option")
+
+    def get_option(self, key: int) -> int:
+        out = ctypes.c_int()
+        _check(self._lib.ts_get_option(self._ctx, int(key), ctypes.byref(out)), "ts_get_option")
+        return out.value
 
     def describe_plan(self) -> str:
         buf = ctypes.create_string_buffer(512)
@@ -221,6 +251,30 @@ class TrotterSuzuki:
         _check(self._lib.ts_overlap(self._ctx, _vp(phi.data_ptr()), out), "ts_overlap")
         return complex(out[0], out[1])
 
+    def correlate(self, alpha: int, j: int, k: int) -> float:
+        out = ctypes.c_double()
+        _check(self._lib.ts_correlate(self._ctx, alpha, j, k, ctypes.byref(out)), "ts_correlate")
+        return out.value
+
+    def total_sz(self) -> float:
+        out = ctypes.c_double()
+        _check(self._lib.ts_total_sz(self._ctx, ctypes.byref(out)), "ts_total_sz")
+        return out.value
+
+    def energy(self) -> float:
+        out = ctypes.c_double()
+        _check(self._lib.ts_energy(self._ctx, ctypes.byref(out)), "ts_energy")
+        return out.value
+
+    def set_random_phase_state(self, up_spin: int, seed: int):
+        _check(self._lib.ts_set_random_phase_state(self._ctx, int(up_spin), int(seed)), "ts_set_random_phase_state")
+
+    def loschmidt_echo(self, tau: float, n_steps: int, order: int = 4):
+        """(M_LE, <psi_0|psi>) after n steps forward and n steps back (eq. 11 with Sigma = 0)."""
+        out = (ctypes.c_double * 3)()
+        _check(self._lib.ts_loschmidt_echo(self._ctx, float(tau), int(n_steps), int(order), out), "ts_loschmidt_echo")
+        return out[0], complex(out[1], out[2])
+
     # ------------------------------------------------------------------ profiling
     def set_profiling(self, enable: bool):
         _check(self._lib.ts_set_profiling(self._ctx, 1 if enable else 0), "ts_set_profiling")
@@ -232,4 +286,7 @@ class TrotterSuzuki:
         l = (ctypes.c_int64 * KC_COUNT)()
         m = (ctypes.c_double * KC_COUNT)()
         _check(self._lib.ts_get_profile(self._ctx, l, m), "ts_get_profile")
-        return {KC_NAMES[i]: {"launches": int(l[i]), "ms": float(m[i])} for i in range(KC_COUNT)}
+        sp = (ctypes.c_double * KC_COUNT)()
+        _check(self._lib.ts_get_profile_passes(self._ctx, sp), "ts_get_profile_passes")
+        return {KC_NAMES[i]: {"launches": int(l[i]), "ms": float(m[i]), "state_passes": float(sp[i])}
+                for i in range(KC_COUNT)}

@@ -15,8 +15,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libts_b200.so")
-SOURCES = ["ts_chunk_cfgH9.cu", "ts_chunk_cfgH8.cu", "ts_chunk_cfgH7.cu", "ts_chunk_cfgH10.cu", "ts_tile_cfgA.cu", "ts_tile_cfgH9.cu", "ts_tile_cfgG.cu", "ts_tile_cfgH10.cu", "ts_tile_cfgH8.cu",
-           "ts_tile_cfgH7.cu", "ts_api.cu", "ts_tile.cu", "ts_naive.cu", "ts_reduce.cu"]
+SOURCES = ["ts_v2_chunk0.cu", "ts_v2_chunk1.cu", "ts_v2_A.cu", "ts_v2_Hs.cu", "ts_v2_Hf.cu", "ts_tile_cfgG.cu", "ts_api.cu",
+           "ts_tile.cu", "ts_naive.cu", "ts_small.cu", "ts_reduce.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -62,32 +62,60 @@ struct Seq {
 int build_plan(ts_ctx* c)
 {
     c->groups.clear();
+    c->use_small = 0;
     const int N = c->N;
     int mode = c->plan_mode;
-    if (mode == TS_PLAN_AUTO) mode = (N >= TS_TILE_LOG2) ? TS_PLAN_TILED : TS_PLAN_NAIVE;
+    if (mode == TS_PLAN_AUTO) {
+        if (N <= TS_SMALL_MAX_N && c->opt_small) { c->use_small = 1; return TS_OK; }
+        mode = (N >= TS_TILE_LOG2) ? TS_PLAN_TILED : TS_PLAN_NAIVE;
+    }
     if (mode == TS_PLAN_NAIVE) return TS_OK;
     if (N < TS_TILE_LOG2) return TS_ERR_ARG;
-    const int s_min = c->run_bits > 0 ? c->run_bits : 3;
-    if (s_min < 1 || s_min > TS_TILE_LOG2 - 1) return TS_ERR_ARG;
-    int mgmax = TS_TILE_LOG2 - s_min;
-    if (c->max_group_bits > 0 && c->max_group_bits < mgmax) mgmax = c->max_group_bits;
     TileGroup A; A.s = TS_TILE_LOG2; A.g0 = TS_TILE_LOG2; A.is_low = 1;
     c->groups.push_back(A);
     const int rem = N - TS_TILE_LOG2;
-    if (rem > 0) {
-        const int ng = (rem + mgmax - 1) / mgmax;
-        int g0 = TS_TILE_LOG2;
-        for (int i = 0; i < ng; ++i) {
-            const int mg = rem / ng + (i < rem % ng ? 1 : 0);    // balanced split: longer runs for everyone
-            TileGroup g; g.s = TS_TILE_LOG2 - mg; g.g0 = g0; g.is_low = 0;
-            c->groups.push_back(g);
-            g0 += mg;
+    std::vector<int> bits;
+    if (!c->explicit_groups.empty()) {
+        // ts_set_plan_groups: the caller (tests, the tuner, a plan file) names the bits of every high group
+        int sum = 0;
+        for (int mg : c->explicit_groups) {
+            if (mg < 1 || mg > TS_TILE_LOG2 - 1) return TS_ERR_ARG;
+            sum += mg;
         }
+        if (sum != rem) return TS_ERR_ARG;
+        bits = c->explicit_groups;
+    } else if (rem > 0) {
+        const int s_min = c->run_bits > 0 ? c->run_bits : 3;
+        if (s_min < 1 || s_min > TS_TILE_LOG2 - 1) return TS_ERR_ARG;
+        int mgmax = TS_TILE_LOG2 - s_min;
+        if (c->max_group_bits > 0 && c->max_group_bits < mgmax) mgmax = c->max_group_bits;
+        int left = rem;
+        if (c->run_bits == 0 && c->max_group_bits == 0 && rem > mgmax) {
+            // default plan: the group right above A takes as many bits as a pass can (9), so that A + that group is a
+            // 32-MiB chunk the L2-blocked triple launch keeps on chip (ts_tile_v2.cuh) at every N >= 22 ...
+            bits.push_back(mgmax);
+            left -= mgmax;
+        }
+        // ... and the bits above are split evenly: the longest runs for every remaining pass
+        const int ng = (left + mgmax - 1) / mgmax;
+        for (int i = 0; i < ng; ++i) bits.push_back(left / ng + (i < left % ng ? 1 : 0));
+    }
+    int g0 = TS_TILE_LOG2;
+    for (int mg : bits) {
+        TileGroup g; g.s = TS_TILE_LOG2 - mg; g.g0 = g0; g.is_low = 0;
+        c->groups.push_back(g);
+        g0 += mg;
     }
     return TS_OK;
 }
 
 bool tiled(const ts_ctx* c) { return !c->groups.empty(); }
+
+int env_int(const char* name, int dflt)
+{
+    const char* v = getenv(name);
+    return v ? atoi(v) : dflt;
+}
 
 int cuda_status(cudaError_t e)
 {
@@ -109,9 +137,10 @@ int ensure_state(ts_ctx* c)
 
 } // namespace
 
-void ts_prof_begin(ts_ctx* c, int kc)
+void ts_prof_begin(ts_ctx* c, int kc, double state_passes)
 {
     c->launches[kc]++;
+    c->tiles_acc[kc] += state_passes;
     if (!c->profiling) return;
     ProfileRec r; r.kc = kc;
     for (cudaEvent_t* e : {&r.e0, &r.e1}) {
@@ -142,7 +171,7 @@ const char* ts_strerror(int s)
     }
 }
 
-const char* ts_version(void) { return "ts_b200 0.1 sm_100a tile=2^12 regs=32amp/thread"; }
+const char* ts_version(void) { return "ts_b200 0.2 sm_100a tile=2^12 regs=32amp/thread kernels=v2(tma-in/out,warp-specialised)+v1"; }
 
 int ts_create(ts_ctx** out, int N, const double* h, const double* J)
 {
@@ -168,25 +197,41 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     }
     c->psi = nullptr; c->owns_psi = 0;
     c->plan_mode = TS_PLAN_AUTO; c->run_bits = 0; c->max_group_bits = 0;
-    c->chunk_log2 = getenv("TS_CHUNK_LOG2") ? atoi(getenv("TS_CHUNK_LOG2")) : 0;
-    c->chunks_per_launch = getenv("TS_CHUNKS_PER_LAUNCH") ? atoi(getenv("TS_CHUNKS_PER_LAUNCH")) : 1;
-    c->pipe_mode = getenv("TS_PIPE") ? atoi(getenv("TS_PIPE")) : 1;
-    c->chunk_mode = getenv("TS_CHUNK3") ? atoi(getenv("TS_CHUNK3")) : 2;
-    c->chunk_max_log2 = getenv("TS_CHUNK3_MAX_LOG2") ? atoi(getenv("TS_CHUNK3_MAX_LOG2")) : 21;
-    c->d_sched = nullptr; c->d_chunk_ctr = nullptr; c->sched_nchunks = 0;
+    // execution options: defaults, overridable once per context from the environment (A/B runs of bench.py) and at
+    // any time through ts_set_option
+    c->opt_kernel = env_int("TS_KERNEL", 1);
+    c->opt_chunk = env_int("TS_CHUNK3", 1);
+    c->opt_chunk_max_log2 = env_int("TS_CHUNK3_MAX_LOG2", 21);
+    c->opt_small = env_int("TS_SMALL", 1);
+    c->opt_diag_source = 0;
+    c->opt_l2_promotion = env_int("TS_L2_PROMOTION", 0);
+    c->opt_max_ctas = 0;
+    c->d_chunk_ctr = nullptr; c->chunk_ctr_cap = 0;
+    c->d_energy[0] = c->d_energy[1] = c->d_energy[2] = nullptr;
     c->tmap_psi = nullptr;
     c->d_red = nullptr; c->red_cap = 0;
+    c->d_trace = nullptr; c->trace_cap = 0;
     c->profiling = 0;
     memset(c->launches, 0, sizeof(c->launches));
     memset(c->ms_acc, 0, sizeof(c->ms_acc));
+    memset(c->tiles_acc, 0, sizeof(c->tiles_acc));
+    if (cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->num_sms < 1) {
+        cudaGetLastError(); delete c; return TS_ERR_CUDA;
+    }
     cudaError_t e = cudaMalloc(&c->d_h, sizeof(c->h));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_Jeff, sizeof(c->Jeff));
     if (e == cudaSuccess) e = cudaMemcpy(c->d_h, c->h, sizeof(c->h), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(c->d_Jeff, c->Jeff, sizeof(c->Jeff), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = ts_tile_init();
+    if (e == cudaSuccess) e = ts_small_init();
     if (e != cudaSuccess) { cudaGetLastError(); ts_destroy(c); return cuda_status(e); }
     int st = build_plan(c);
     if (st != TS_OK) { ts_destroy(c); return st; }
+    const char* pf = getenv("TS_PLAN_FILE");       // a tuned plan (paper_1305_0036_b200/tuner.py) for this size, if any
+    if (pf && *pf) {
+        st = ts_load_plan_file(c, pf);
+        if (st != TS_OK) { ts_destroy(c); return st; }
+    }
     *out = c;
     return TS_OK;
 }
@@ -198,9 +243,10 @@ int ts_destroy(ts_ctx* c)
     if (c->d_h) cudaFree(c->d_h);
     if (c->d_Jeff) cudaFree(c->d_Jeff);
     ts_tile_free_tables(c);
+    ts_naive_free_stored(c);
     if (c->d_red) cudaFree(c->d_red);
-    if (c->d_sched) cudaFree(c->d_sched);
     if (c->d_chunk_ctr) cudaFree(c->d_chunk_ctr);
+    if (c->d_trace) cudaFree(c->d_trace);
     for (auto& r : c->recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto& e : c->ev_pool) cudaEventDestroy(e);
     delete c;
@@ -271,12 +317,118 @@ int ts_set_plan(ts_ctx* c, int mode, int run_bits, int max_group_bits)
 {
     if (!c || mode < TS_PLAN_AUTO || mode > TS_PLAN_TILED || run_bits < 0 || max_group_bits < 0) return TS_ERR_ARG;
     const int om = c->plan_mode, orb = c->run_bits, omg = c->max_group_bits;
+    const std::vector<int> oeg = c->explicit_groups;
     c->plan_mode = mode; c->run_bits = run_bits; c->max_group_bits = max_group_bits;
+    c->explicit_groups.clear();
     cudaStreamSynchronize(c->stream);
     ts_tile_free_tables(c);          // tables depend on the group geometry
     c->tmaps.clear();
     int st = build_plan(c);
-    if (st != TS_OK) { c->plan_mode = om; c->run_bits = orb; c->max_group_bits = omg; build_plan(c); }
+    if (st != TS_OK) { c->plan_mode = om; c->run_bits = orb; c->max_group_bits = omg; c->explicit_groups = oeg; build_plan(c); }
+    return st;
+}
+
+int ts_set_plan_groups(ts_ctx* c, int n_high, const int* high_bits)
+{
+    if (!c || n_high < 0 || (n_high > 0 && !high_bits) || c->N < TS_TILE_LOG2) return TS_ERR_ARG;
+    if ((n_high == 0) != (c->N == TS_TILE_LOG2)) return TS_ERR_ARG;
+    const int om = c->plan_mode;
+    const std::vector<int> oeg = c->explicit_groups;
+    c->plan_mode = TS_PLAN_TILED;
+    c->explicit_groups.assign(high_bits, high_bits + n_high);
+    cudaStreamSynchronize(c->stream);
+    ts_tile_free_tables(c);
+    c->tmaps.clear();
+    int st = build_plan(c);
+    if (st != TS_OK) { c->plan_mode = om; c->explicit_groups = oeg; build_plan(c); }
+    return st;
+}
+
+int ts_set_option(ts_ctx* c, int key, int value)
+{
+    if (!c) return TS_ERR_ARG;
+    switch (key) {
+    case TS_OPT_KERNEL: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_kernel = value; break;
+    case TS_OPT_CHUNK: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_chunk = value; break;
+    case TS_OPT_CHUNK_MAX_LOG2: if (value < TS_TILE_LOG2 + 1 || value > 26) return TS_ERR_ARG; c->opt_chunk_max_log2 = value; break;
+    case TS_OPT_L2_PROMOTION: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_l2_promotion = value; c->tmaps.clear(); break;
+    case TS_OPT_MAX_CTAS: if (value < 0) return TS_ERR_ARG; c->opt_max_ctas = value; break;
+    case TS_OPT_DIAG_SOURCE:
+        if (value < 0 || value > 1) return TS_ERR_ARG;
+        c->opt_diag_source = value;
+        if (!value) { cudaStreamSynchronize(c->stream); ts_naive_free_stored(c); }
+        break;
+    case TS_OPT_SMALL:
+        if (value < 0 || value > 1) return TS_ERR_ARG;
+        c->opt_small = value;
+        cudaStreamSynchronize(c->stream);
+        ts_tile_free_tables(c);
+        c->tmaps.clear();
+        return build_plan(c);
+    default: return TS_ERR_ARG;
+    }
+    // phase tables are keyed by the kernel family that reads them, so nothing cached goes stale
+    return TS_OK;
+}
+
+int ts_get_option(ts_ctx* c, int key, int* value)
+{
+    if (!c || !value) return TS_ERR_ARG;
+    switch (key) {
+    case TS_OPT_KERNEL: *value = c->opt_kernel; break;
+    case TS_OPT_CHUNK: *value = c->opt_chunk; break;
+    case TS_OPT_CHUNK_MAX_LOG2: *value = c->opt_chunk_max_log2; break;
+    case TS_OPT_L2_PROMOTION: *value = c->opt_l2_promotion; break;
+    case TS_OPT_SMALL: *value = c->opt_small; break;
+    case TS_OPT_DIAG_SOURCE: *value = c->opt_diag_source; break;
+    case TS_OPT_MAX_CTAS: *value = c->opt_max_ctas; break;
+    default: return TS_ERR_ARG;
+    }
+    return TS_OK;
+}
+
+// Plan file (the tuned sequence of rotations per N "stored in a file"): text, one line per system size,
+//     N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 l2_promotion=0
+// `groups` = bits of every high group, bottom to top (ts_set_plan_groups); the other keys are ts_set_option values and
+// may be omitted.  Lines starting with '#' are comments.  Returns TS_OK and leaves the context untouched when the file
+// has no line for this N.
+int ts_load_plan_file(ts_ctx* c, const char* path)
+{
+    if (!c || !path) return TS_ERR_ARG;
+    FILE* f = fopen(path, "r");
+    if (!f) return TS_ERR_ARG;
+    char line[512];
+    int st = TS_OK;
+    while (fgets(line, sizeof line, f)) {
+        if (line[0] == '#') continue;
+        int n = -1;
+        std::vector<int> groups;
+        int kernel = -1, chunk = -1, cmax = -1, prom = -1;
+        bool have_groups = false;
+        for (char* tok = strtok(line, " \t\r\n"); tok; tok = strtok(nullptr, " \t\r\n")) {
+            if (!strncmp(tok, "N=", 2)) n = atoi(tok + 2);
+            else if (!strncmp(tok, "groups=", 7)) {
+                have_groups = true;
+                for (const char* p = tok + 7; *p;) {
+                    groups.push_back(atoi(p));
+                    while (*p && *p != ',') ++p;
+                    if (*p == ',') ++p;
+                }
+            }
+            else if (!strncmp(tok, "kernel=", 7)) kernel = atoi(tok + 7);
+            else if (!strncmp(tok, "chunk=", 6)) chunk = atoi(tok + 6);
+            else if (!strncmp(tok, "chunk_max_log2=", 15)) cmax = atoi(tok + 15);
+            else if (!strncmp(tok, "l2_promotion=", 13)) prom = atoi(tok + 13);
+        }
+        if (n != c->N) continue;
+        if (kernel >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_KERNEL, kernel);
+        if (chunk >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_CHUNK, chunk);
+        if (cmax >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_CHUNK_MAX_LOG2, cmax);
+        if (prom >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_L2_PROMOTION, prom);
+        if (have_groups && st == TS_OK && c->N >= TS_TILE_LOG2 + 1) st = ts_set_plan_groups(c, (int)groups.size(), groups.data());
+        break;
+    }
+    fclose(f);
     return st;
 }
 
@@ -285,7 +437,10 @@ int ts_describe_plan(ts_ctx* c, char* buf, int buflen)
     if (!c || !buf || buflen < 1) return TS_ERR_ARG;
     std::string s;
     char tmp[128];
-    if (!tiled(c)) {
+    if (c->use_small) {
+        snprintf(tmp, sizeof tmp, "small: N=%d, one CTA, state and energy tables in shared memory, one launch per ts_evolve", c->N);
+        s = tmp;
+    } else if (!tiled(c)) {
         snprintf(tmp, sizeof tmp, "naive: N=%d, %d one-bit rotation launches + 1 diagonal launch per sweep", c->N, c->N);
         s = tmp;
     } else {
@@ -296,6 +451,13 @@ int ts_describe_plan(ts_ctx* c, char* buf, int buflen)
         for (const TileGroup& t : c->groups) {
             if (t.is_low) snprintf(tmp, sizeof tmp, " A[spins 0..11]");
             else snprintf(tmp, sizeof tmp, " H[spins %d..%d, run 2^%d]", t.g0, t.g0 + TS_TILE_LOG2 - t.s - 1, t.s);
+            s += tmp;
+        }
+        snprintf(tmp, sizeof tmp, "; kernels=%s", c->opt_kernel ? "v2" : "v1");
+        s += tmp;
+        if (ts_tile_chunk_supported(c, 1, SW_YDAG, SW_Y)) {
+            const TileGroup& t = c->groups[1];
+            snprintf(tmp, sizeof tmp, "; L2-blocked triple launch on chunks of 2^%d", t.g0 + TS_TILE_LOG2 - t.s);
             s += tmp;
         }
     }
@@ -311,6 +473,7 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
     const Seq q(order, c->N, tau, n_steps);
     cudaError_t e = cudaSuccess;
 
+    if (c->use_small) return cuda_status(ts_small_evolve(c, tau, n_steps, order));
     if (!tiled(c)) {
         e = ts_naive_diag(c, q.diag(0));
         for (int64_t i = 1; i <= q.M && e == cudaSuccess; ++i) {
@@ -320,86 +483,61 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
         return cuda_status(e);
     }
 
-    // ---- pass list: one entry per HBM round trip (or per L2 round trip inside a blocked run)
+    // ---- passes are generated sweep by sweep (the paper's runs are 5e5 .. 5e6 steps: no list of them
+    // is ever materialised) and executed through a three-entry window in which the pattern
+    //     [H1 single ka] [A fused ka . D . kb] [H1 single kb]   ->   one L2-blocked launch (ts_tile_v2.cuh)
+    // is recognised.
     struct Pass { int gi, k1, k2; DiagOp d; };
-    std::vector<Pass> passes;
-    auto push = [&](int gi, int k1, const DiagOp* d, int k2) {
-        Pass ps; ps.gi = gi; ps.k1 = k1; ps.k2 = k2;
-        if (d) ps.d = *d; else ps.d.present = 0;
-        passes.push_back(ps);
-    };
     const int g = (int)c->groups.size();
-    for (int64_t i = 1; i <= q.M; ++i) {
-        const bool fwd = (i & 1);
-        if (g == 1) {
-            const DiagOp d0 = q.diag(i - 1);
-            push(0, SW_NONE, &d0, q.kind(i));
-            if (i == q.M) { const DiagOp dm = q.diag(q.M); push(0, SW_NONE, &dm, SW_NONE); }
-            continue;
-        }
-        for (int pos = 0; pos < g; ++pos) {
-            const int gi = fwd ? pos : g - 1 - pos;
-            const bool first = (pos == 0), last = (pos == g - 1);
-            if (first && i > 1) continue;                              // done by the previous fused pass
-            if (last && i < q.M) {                                     // sweep i . D_i . sweep i+1 on the same group
-                const DiagOp d = q.diag(i);
-                push(gi, q.kind(i), &d, q.kind(i + 1));
-            } else if (first && i == 1) {
-                const DiagOp d = q.diag(0);
-                push(gi, SW_NONE, &d, q.kind(1));
-            } else if (last && i == q.M) {
-                const DiagOp d = q.diag(q.M);
-                push(gi, q.kind(i), &d, SW_NONE);
+    int64_t sweep = 1;                 // next sweep to expand
+    int pos = 0;                       // next position within it
+    Pass win[4];
+    int nwin = 0;
+    auto refill = [&]() {
+        while (nwin < 3 && sweep <= q.M) {
+            const int64_t i = sweep;
+            Pass ps; ps.d.present = 0; ps.gi = 0; ps.k1 = SW_NONE; ps.k2 = SW_NONE;
+            bool emit = true;
+            if (g == 1) {
+                if (pos == 0) { ps.d = q.diag(i - 1); ps.k2 = q.kind(i); }
+                else { ps.d = q.diag(q.M); }                                // trailing diagonal after the last sweep
+                ++pos;
+                if (pos > (i == q.M ? 1 : 0)) { ++sweep; pos = 0; }
             } else {
-                push(gi, q.kind(i), nullptr, SW_NONE);
+                const bool fwd = (i & 1);
+                const bool first = (pos == 0), last = (pos == g - 1);
+                ps.gi = fwd ? pos : g - 1 - pos;
+                if (first && i > 1) emit = false;                              // done by the previous fused pass
+                else if (last && i < q.M) { ps.k1 = q.kind(i); ps.d = q.diag(i); ps.k2 = q.kind(i + 1); }
+                else if (first && i == 1) { ps.d = q.diag(0); ps.k2 = q.kind(1); }
+                else if (last && i == q.M) { ps.k1 = q.kind(i); ps.d = q.diag(q.M); }
+                else ps.k1 = q.kind(i);
+                if (++pos == g) { ++sweep; pos = 0; }
             }
+            if (emit) win[nwin++] = ps;
         }
-    }
-
-    auto launch = [&](const Pass& ps, uint64_t tile_base, uint64_t tile_count) -> cudaError_t {
-        const DiagTables* tb = nullptr;
-        if (ps.d.present) {
-            cudaError_t ee = ts_tile_get_tables(c, ps.d, ps.gi, &tb);
-            if (ee != cudaSuccess) return ee;
-        }
-        return ts_tile_pass(c, ps.gi, ps.k1, tb, ps.k2, tile_base, tile_count);
     };
-
-    // ---- execution.  L2 blocking: consecutive passes whose groups all lie below spin
-    // `chunk_log2` act inside aligned chunks of 2^chunk_log2 amplitudes (closed-set argument of P:141 applied to the
-    // chunk), so such a run is executed chunk window by chunk window: the window is read from HBM by the first pass,
-    // stays in the 126 MB L2 for the passes in between and is written back once.
-    const int C = c->chunk_log2;
-    const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
-    auto top_spin = [&](int gi) { const TileGroup& t = c->groups[gi]; return t.is_low ? TS_TILE_LOG2 - 1 : t.g0 + TS_TILE_LOG2 - t.s - 1; };
-    size_t ip = 0;
-    while (ip < passes.size() && e == cudaSuccess) {
-        // [H single ka] [A fused ka . D . kb] [H single kb]  ->  one L2-blocked launch (ts_tile_chunk.cuh)
-        if (ip + 2 < passes.size()) {
-            const Pass &p0 = passes[ip], &p1 = passes[ip + 1], &p2 = passes[ip + 2];
+    for (;;) {
+        refill();
+        if (nwin == 0 || e != cudaSuccess) break;
+        int used = 1;
+        if (nwin >= 3) {
+            const Pass &p0 = win[0], &p1 = win[1], &p2 = win[2];
             if (p0.gi == p2.gi && p1.gi == 0 && p0.k2 == SW_NONE && !p0.d.present && p2.k2 == SW_NONE && !p2.d.present &&
                 p1.d.present && p1.k1 == p0.k1 && p1.k2 == p2.k1 && ts_tile_chunk_supported(c, p0.gi, p1.k1, p1.k2)) {
-                const DiagTables* tb = nullptr;
-                e = ts_tile_get_tables(c, p1.d, 0, &tb);
-                if (e == cudaSuccess) e = ts_tile_chunk_triple(c, p0.gi, p1.k1, tb, p1.k2);
-                ip += 3;
-                continue;
+                e = ts_tile_chunk_triple(c, p0.gi, p1.k1, p1.d, p1.k2);
+                if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources || e == cudaErrorNotSupported) {
+                    cudaGetLastError();          // not all CTAs can be co-resident here (MPS, a shared GPU): run the
+                    c->opt_chunk = 0;            // three passes one by one from now on
+                    e = cudaSuccess;
+                } else {
+                    used = 3;
+                }
             }
         }
-        size_t jp = ip;
-        if (C > 0 && C < c->N)
-            while (jp < passes.size() && top_spin(passes[jp].gi) < C) ++jp;
-        if (jp - ip >= 2) {
-            const uint64_t win = ((uint64_t)1 << (C - TS_TILE_LOG2)) * (uint64_t)(c->chunks_per_launch > 0 ? c->chunks_per_launch : 1);
-            for (uint64_t tb0 = 0; tb0 < ntiles && e == cudaSuccess; tb0 += win) {
-                const uint64_t cnt = (ntiles - tb0 < win) ? ntiles - tb0 : win;
-                for (size_t k = ip; k < jp && e == cudaSuccess; ++k) e = launch(passes[k], tb0, cnt);
-            }
-            ip = jp;
-        } else {
-            e = launch(passes[ip], 0, 0);
-            ++ip;
-        }
+        if (used == 1) e = ts_tile_pass(c, win[0].gi, win[0].k1, win[0].d.present ? &win[0].d : nullptr, win[0].k2);
+        for (int k = used; k < nwin; ++k) win[k - used] = win[k];
+        nwin -= used;
     }
     return cuda_status(e);
 }
@@ -410,9 +548,16 @@ int ts_evolve_observe(ts_ctx* c, double tau, int64_t n_steps, int order, int alp
     if (alpha == TS_Z ? (j < -1 || j >= c->N) : (j < 0 || j >= c->N)) return TS_ERR_ARG;
     if (!c->psi) return TS_ERR_NOSTATE;
     if (n_steps == 0) return TS_OK;
-    double* d_trace = nullptr;
-    cudaError_t e = cudaMalloc(&d_trace, sizeof(double) * TS_TRACE_STRIDE * (size_t)n_steps);
-    if (e != cudaSuccess) { cudaGetLastError(); return TS_ERR_NOMEM; }
+    cudaError_t e = cudaSuccess;
+    const size_t need = (size_t)TS_TRACE_STRIDE * (size_t)n_steps;
+    if (c->trace_cap < need) {
+        if (c->d_trace) { cudaStreamSynchronize(c->stream); cudaFree(c->d_trace); }
+        c->d_trace = nullptr; c->trace_cap = 0;
+        e = cudaMalloc(&c->d_trace, sizeof(double) * need);
+        if (e != cudaSuccess) { cudaGetLastError(); return TS_ERR_NOMEM; }
+        c->trace_cap = need;
+    }
+    double* d_trace = c->d_trace;
     int st = TS_OK;
     for (int64_t k = 0; k < n_steps && st == TS_OK; ++k) {
         st = ts_evolve(c, tau, 1, order);
@@ -427,7 +572,6 @@ int ts_evolve_observe(ts_ctx* c, double tau, int64_t n_steps, int order, int alp
     } else {
         cudaStreamSynchronize(c->stream);
     }
-    cudaFree(d_trace);
     if (st != TS_OK) return st;
     for (int64_t k = 0; k < n_steps; ++k) {
         const double* row = host.data() + (size_t)k * TS_TRACE_STRIDE;
@@ -460,6 +604,8 @@ int ts_expect_all(ts_ctx* c, int alpha, double* out)
     if (!c || !out || alpha < TS_X || alpha > TS_Z) return TS_ERR_ARG;
     if (!c->psi) return TS_ERR_NOSTATE;
     if (alpha == TS_Z) return cuda_status(ts_reduce_expect_z_all(c, out));
+    if (tiled(c))       // one pass per bit group of the plan (every tile holds both members of the group's pairs)
+        return cuda_status(ts_reduce_expect_xy_all(c, alpha == TS_X ? out : nullptr, alpha == TS_Y ? out : nullptr));
     for (int j = 0; j < c->N; ++j) {
         cudaError_t e = ts_reduce_expect_xy(c, alpha, j, out + j);
         if (e != cudaSuccess) return cuda_status(e);
@@ -479,6 +625,97 @@ int ts_overlap(ts_ctx* c, const void* dev_phi, double* out)
     if (!c || !out || !dev_phi) return TS_ERR_ARG;
     if (!c->psi) return TS_ERR_NOSTATE;
     return cuda_status(ts_reduce_overlap(c, (const double2*)dev_phi, out));
+}
+
+int ts_correlate(ts_ctx* c, int alpha, int j, int k, double* out)
+{
+    if (!c || !out || alpha < TS_X || alpha > TS_Z || j < 0 || j >= c->N || k < 0 || k >= c->N || j == k) return TS_ERR_ARG;
+    if (!c->psi) return TS_ERR_NOSTATE;
+    return cuda_status(ts_reduce_corr(c, alpha, j, k, out));
+}
+
+int ts_total_sz(ts_ctx* c, double* out)
+{
+    if (!c || !out) return TS_ERR_ARG;
+    if (!c->psi) return TS_ERR_NOSTATE;
+    double v[TS_MAX_N];
+    cudaError_t e = ts_reduce_expect_z_all(c, v);
+    if (e != cudaSuccess) return cuda_status(e);
+    double s = 0.0;
+    for (int j = 0; j < c->N; ++j) s += v[j];
+    *out = s;
+    return TS_OK;
+}
+
+namespace {
+
+// One global rotation (sweep) of the state, optionally followed by the exact scaling 2^scale_pow: every group of the
+// plan once (tiled), or one launch per spin (naive / small-N contexts).
+cudaError_t apply_sweep(ts_ctx* c, int kind, int scale_pow)
+{
+    cudaError_t e = cudaSuccess;
+    DiagOp d; d.present = (scale_pow != 0); d.alpha = TS_Z; d.t = 0.0; d.scale_pow = scale_pow;
+    if (!tiled(c)) {
+        for (int j = 0; j < c->N && e == cudaSuccess; ++j) e = ts_naive_rotate(c, j, kind);
+        if (e == cudaSuccess && d.present) e = ts_naive_diag(c, d);
+        return e;
+    }
+    const int g = (int)c->groups.size();
+    for (int gi = 0; gi < g && e == cudaSuccess; ++gi)
+        e = ts_tile_pass(c, gi, kind, (gi == g - 1 && d.present) ? &d : nullptr, SW_NONE);
+    return e;
+}
+
+} // namespace
+
+int ts_energy(ts_ctx* c, double* out)
+{
+    if (!c || !out) return TS_ERR_ARG;
+    if (!c->psi) return TS_ERR_NOSTATE;
+    // <H> = <H_z> + <H_x> + <H_y>;  <psi|H_x|psi> = sum_k E_x(k) |(Y^dag psi)_k|^2 and <psi|H_y|psi> = sum_k E_y(k)
+    // |(X^dag psi)_k|^2 (eq. 7, 10: P:81-84), the unnormalised sweeps carrying a factor 2^N in |.|^2.
+    double ez = 0.0, ex = 0.0, ey = 0.0;
+    cudaError_t e = ts_reduce_energy_diag(c, TS_Z, &ez);
+    if (e == cudaSuccess) e = apply_sweep(c, SW_YDAG, 0);
+    if (e == cudaSuccess) e = ts_reduce_energy_diag(c, TS_X, &ex);
+    if (e == cudaSuccess) e = apply_sweep(c, SW_Y, -c->N);           // back: Y Y^dag = 2^N, removed exactly
+    if (e == cudaSuccess) e = apply_sweep(c, SW_XDAG, 0);
+    if (e == cudaSuccess) e = ts_reduce_energy_diag(c, TS_Y, &ey);
+    if (e == cudaSuccess) e = apply_sweep(c, SW_X, -c->N);
+    if (e != cudaSuccess) return cuda_status(e);
+    const double sc = ldexp(1.0, -c->N);
+    *out = ez + sc * (ex + ey);
+    return TS_OK;
+}
+
+int ts_set_random_phase_state(ts_ctx* c, int up_spin, uint64_t seed)
+{
+    if (!c || up_spin < 0 || up_spin >= c->N) return TS_ERR_ARG;
+    int st = ensure_state(c);
+    if (st != TS_OK) return st;
+    return cuda_status(ts_fill_random_phase(c, up_spin, seed));
+}
+
+int ts_loschmidt_echo(ts_ctx* c, double tau, int64_t n_steps, int order, double* out)
+{
+    if (!c || !out || !isfinite(tau) || n_steps < 0 || (order != 2 && order != 4)) return TS_ERR_ARG;
+    if (!c->psi) return TS_ERR_NOSTATE;
+    double2* psi0 = nullptr;
+    const size_t bytes = sizeof(double2) << c->N;
+    if (cudaMalloc(&psi0, bytes) != cudaSuccess) { cudaGetLastError(); return TS_ERR_NOMEM; }
+    cudaError_t e = cudaMemcpyAsync(psi0, c->psi, bytes, cudaMemcpyDeviceToDevice, c->stream);
+    int st = cuda_status(e);
+    if (st == TS_OK) st = ts_evolve(c, tau, n_steps, order);
+    if (st == TS_OK) st = ts_evolve(c, -tau, n_steps, order);
+    double ov[2] = {0.0, 0.0};
+    if (st == TS_OK) st = cuda_status(ts_reduce_overlap(c, psi0, ov));
+    else cudaStreamSynchronize(c->stream);
+    cudaFree(psi0);
+    if (st != TS_OK) return st;
+    out[0] = ov[0] * ov[0] + ov[1] * ov[1];
+    out[1] = ov[0];
+    out[2] = ov[1];
+    return TS_OK;
 }
 
 int ts_set_profiling(ts_ctx* c, int enable)
@@ -505,6 +742,13 @@ int ts_get_profile(ts_ctx* c, int64_t* launches, double* ms)
     return TS_OK;
 }
 
+int ts_get_profile_passes(ts_ctx* c, double* state_passes)
+{
+    if (!c || !state_passes) return TS_ERR_ARG;
+    for (int k = 0; k < TS_KC_COUNT; ++k) state_passes[k] = c->tiles_acc[k];
+    return TS_OK;
+}
+
 int ts_reset_profile(ts_ctx* c)
 {
     if (!c) return TS_ERR_ARG;
@@ -512,6 +756,7 @@ int ts_reset_profile(ts_ctx* c)
     int st = ts_get_profile(c, l, m);      // drains pending records
     memset(c->launches, 0, sizeof(c->launches));
     memset(c->ms_acc, 0, sizeof(c->ms_acc));
+    memset(c->tiles_acc, 0, sizeof(c->tiles_acc));
     return st;
 }
 

@@ -1,8 +1,8 @@
 // ts_internal.h -- shared declarations of the CUDA path (host side).  Not part of the public ABI.
 //
-// Layers: ts_api.cu (C ABI, context, sequencer, plan) -> launchers in ts_tile.cu
-// (tile passes + phase tables), ts_naive.cu (one-bit rotations, brute-force diagonal), ts_reduce.cu (observables).
-// Nothing here is shared with oracle/.
+// Layers: ts_api.cu (C ABI, context, sequencer, plan) -> launchers in ts_tile.cu (tile passes + phase
+// tables), ts_naive.cu (one-bit rotations, brute-force diagonal, stored-phase diagonal), ts_small.cu (single-CTA
+// path for N <= 12), ts_reduce.cu (observables).  Nothing here is shared with oracle/.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -38,9 +38,10 @@ struct TileGroup {
     int is_low;   // group A: butterflies all 12 tile bits; otherwise the 12 - s group bits
 };
 
-// Phase tables of one (diagonal kind, tile group), see ts_tile_kernel.cuh.  Built on first use, cached in the context.
+// Phase tables of one (diagonal kind, tile group, kernel family), see ts_tile_kernel.cuh.  Built on first use, cached
+// in the context; handles stay valid until ts_tile_free_tables.
 struct DiagTables {
-    int alpha, scale_pow, group;
+    int alpha, scale_pow, group, layout;   // layout: 0 = k_tile_pass register layout, 1 = v2 (ts_tile_v2.cuh)
     double t;
     double2* d_thread;       // device: TT[128] followed by WT[5][128]
     double2* d_tile_phase;   // device: [ntiles][32]
@@ -59,6 +60,7 @@ struct ProfileRec { int kc; cudaEvent_t e0, e1; };
 struct ts_ctx {
     int N;
     int device;
+    int num_sms;
     cudaStream_t stream;
     double h[3][TS_MAX_N];
     double Jeff[3][TS_MAX_N][TS_MAX_N];   // symmetric, zero diagonal: Jeff[j][k] = J[j][k] + J[k][j]  (A1)
@@ -68,52 +70,73 @@ struct ts_ctx {
     int owns_psi;
     // plan
     int plan_mode, run_bits, max_group_bits;
-    int chunk_log2, chunks_per_launch;   // L2 blocking (0 = off)
-    int chunk_mode, chunk_max_log2;      // L2-blocked triple launches (ts_tile_chunk.cuh): on/off, largest chunk (log2 amplitudes)
-    uint32_t* d_sched;                   // job-block order of the triple launch, for sched_nchunks chunks
-    unsigned int* d_chunk_ctr;           // ticket + done counters
-    uint32_t sched_nchunks;
-    int pipe_mode;                       // 1: persistent TMA-pipelined tile kernels (ts_tile_pipe.cuh), 0: one CTA per tile
+    std::vector<int> explicit_groups;    // ts_set_plan_groups: bits of each high group, bottom to top (empty: automatic)
+    std::vector<TileGroup> groups;
+    int use_small;                       // N <= 12 under TS_PLAN_AUTO: the single-CTA path (ts_small.cu)
+    // execution options (ts_set_option)
+    int opt_kernel;                      // 1: v2 pipelined kernels where the geometry allows, 0: k_tile_pass only
+    int opt_chunk;                       // 1: L2-blocked triple launches
+    int opt_chunk_max_log2;              // largest chunk (log2 amplitudes)
+    int opt_small;                       // 1: single-CTA path for N <= 12
+    int opt_diag_source;                 // 0: factorised on-the-fly tables, 1: stored 2^N phase vectors, naive plan only
+    int opt_l2_promotion;                // tensor-map L2 promotion of the high groups: 0 none, 1 128 B, 2 256 B
+    int opt_max_ctas;                    // upper bound on the persistent kernels' grid (0: one CTA per SM)
+    unsigned int* d_chunk_ctr;           // done counters of the triple launch
+    size_t chunk_ctr_cap;
     std::vector<TensorMapSlot> tmaps;    // per group, for the bound state pointer tmap_psi
     void* tmap_psi;
-    std::vector<TileGroup> groups;
     // phase tables, built on demand and cached (invalidated when the plan changes)
-    std::vector<DiagTables> tabs;
+    std::vector<DiagTables*> tabs;
+    double* d_energy[3];                 // the stored energy vectors E_x, E_y, E_z of the table variant, built on demand
     // reduction scratch
     double* d_red;
     size_t red_cap;   // in doubles
+    double* d_trace;  // ts_evolve_observe rows
+    size_t trace_cap;
     // profiling
     int profiling;
     int64_t launches[TS_KC_COUNT];
     double ms_acc[TS_KC_COUNT];
+    double tiles_acc[TS_KC_COUNT];       // tile passes x tiles performed per class, in units of whole-state passes
     std::vector<ProfileRec> recs;
     std::vector<cudaEvent_t> ev_pool;
 };
 
-// ---- profiling helpers (ts_api.cu)
-void ts_prof_begin(ts_ctx* c, int kc);
+// ---- profiling helpers (ts_api.cu).  `state_passes`: tile passes over the whole state this launch performs
+// (1 for a tile pass, 3 for a triple launch, N-bit fractions for the rest are not counted: 0).
+void ts_prof_begin(ts_ctx* c, int kc, double state_passes = 0.0);
 void ts_prof_end(ts_ctx* c);
 
 // ---- naive path (ts_naive.cu)
 cudaError_t ts_naive_rotate(ts_ctx* c, int j, int kind);
 cudaError_t ts_naive_diag(ts_ctx* c, const DiagOp& d);
+void ts_naive_free_stored(ts_ctx* c);
+
+// ---- single-CTA path for small N (ts_small.cu): the whole ts_evolve call in one launch
+#define TS_SMALL_MAX_N 12
+cudaError_t ts_small_evolve(ts_ctx* c, double tau, int64_t n_steps, int order);
+cudaError_t ts_small_init(void);
 
 // ---- tiled path (ts_tile.cu)
-cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, const DiagTables** out);
+cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, int layout, const DiagTables** out);
 void ts_tile_free_tables(ts_ctx* c);
-// tile_count = 0: all tiles; otherwise the window [tile_base, tile_base + tile_count)
-cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagTables* tabs /*or NULL*/, int kind2,
-                         uint64_t tile_base, uint64_t tile_count);
+// which phase-table layout the pass (group, kind1, kind2) will use (0 / 1), i.e. which kernel family runs it
+int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2);
+cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d /*or NULL*/, int kind2);
 bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb);
-// [H(gh) single ka] [A fused ka . D(tabs) . kb] [H(gh) single kb] in one L2-blocked launch
-cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagTables* tabs, int kb);
-cudaError_t ts_tile_init(void);   // registers the kernels, sets max dynamic shared memory on all of them
+// [H(gh) single ka] [A fused ka . D . kb] [H(gh) single kb] in one L2-blocked launch
+cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int kb);
+cudaError_t ts_tile_init(void);   // registers the kernels, sets max dynamic shared memory on all of them (once per process)
 
 // ---- reductions (ts_reduce.cu)
 cudaError_t ts_reduce_expect_z_all(ts_ctx* c, double* out_host /*[N]*/);
 cudaError_t ts_reduce_expect_xy(ts_ctx* c, int alpha, int j, double* out_host);
+cudaError_t ts_reduce_expect_xy_all(ts_ctx* c, double* out_x /*[N] or NULL*/, double* out_y /*[N] or NULL*/);   // tiled plans
 cudaError_t ts_reduce_norm2(ts_ctx* c, double* out_host);
 cudaError_t ts_reduce_overlap(ts_ctx* c, const double2* phi, double* out_host /*[2]*/);
+cudaError_t ts_reduce_corr(ts_ctx* c, int alpha, int j, int k, double* out_host);   // <S^a_j S^a_k>
+cudaError_t ts_reduce_energy_diag(ts_ctx* c, int alpha, double* out_host);   // sum_k E_alpha(k) |c_k|^2 of the state AS STORED
 cudaError_t ts_fill_basis(ts_ctx* c, uint64_t k);
+cudaError_t ts_fill_random_phase(ts_ctx* c, int up_spin, uint64_t seed);
 #define TS_TRACE_STRIDE (TS_MAX_N + 1)
 cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row /*[TS_TRACE_STRIDE]*/);

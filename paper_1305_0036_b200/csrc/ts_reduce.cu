@@ -3,6 +3,8 @@
 //   <S^z_j> = 1/2 sum_k (2 bit_j(k) - 1) |c_k|^2
 //   <S^x_j> = sum_{k: bit_j = 0} Re( conj(c_{k + 2^j}) c_k ),   <S^y_j> = same with Im
 // Deterministic two-stage FP64 reduction: fixed grid, per-block partials, then one block sums them in index order.
+#include <math.h>
+
 #include "ts_internal.h"
 
 namespace {
@@ -81,6 +83,56 @@ __global__ void __launch_bounds__(RB) k_pair_xy(const double2* __restrict__ psi,
     if (threadIdx.x == 0) partial[(size_t)blockIdx.x * MAXV + 1] = r;
 }
 
+// All sites of one bit group in ONE pass (the tile geometry of the time step: a closed tile holds both members of
+// every pair of the group's spins).  A CTA stages tiles of 2^12 amplitudes in shared memory (f < s <-> spin f,
+// f >= s <-> spin g0 + f - s) and accumulates, for each of the nb spins on tile bits f0 .. f0 + nb - 1,
+//   sum over pairs (c0: bit = 0, c1: bit = 1) of conj(c1) c0   ->   Re = <S^x>, Im = <S^y>      (reading A15)
+// partial[blockIdx][2 i], [2 i + 1] = Re, Im for tile bit f0 + i.
+constexpr int XG_T = 256;
+__global__ void __launch_bounds__(XG_T) k_pair_xy_group(const double2* __restrict__ psi, uint64_t ntiles, int s, int g0, int f0, int nb,
+                                                       double* __restrict__ partial)
+{
+    extern __shared__ double2 tile[];      // 4096 amplitudes
+    __shared__ double sh[RB / 32];
+    double ax[TS_TILE_LOG2], ay[TS_TILE_LOG2];
+#pragma unroll
+    for (int i = 0; i < TS_TILE_LOG2; ++i) { ax[i] = 0.0; ay[i] = 0.0; }
+    const int t = threadIdx.x;
+    const int nmid = g0 - s;
+    const uint64_t runmask = ((uint64_t)1 << s) - 1;
+    for (uint64_t tau = blockIdx.x; tau < ntiles; tau += gridDim.x) {
+        const uint64_t base = ((tau & (((uint64_t)1 << nmid) - 1)) << s) | ((tau >> nmid) << (g0 + TS_TILE_LOG2 - s));
+        __syncthreads();                   // the previous tile has been read by everyone
+        for (int f = t; f < (1 << TS_TILE_LOG2); f += XG_T)
+            tile[f] = psi[base + (((uint64_t)f & runmask) | (((uint64_t)f >> s) << g0))];
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < TS_TILE_LOG2; ++i) {
+            if (i < nb) {
+                const int b = f0 + i;
+                const int low = (1 << b) - 1;
+                double sx = 0.0, sy = 0.0;
+                for (int q = t; q < (1 << (TS_TILE_LOG2 - 1)); q += XG_T) {
+                    const int k0 = ((q & ~low) << 1) | (q & low);
+                    const double2 c0 = tile[k0], c1 = tile[k0 | (1 << b)];
+                    sx += c1.x * c0.x + c1.y * c0.y;
+                    sy += c1.x * c0.y - c1.y * c0.x;
+                }
+                ax[i] += sx; ay[i] += sy;
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < TS_TILE_LOG2; ++i) {
+        if (i < nb) {
+            double r = block_sum(ax[i], sh);
+            if (t == 0) partial[(size_t)blockIdx.x * MAXV + 2 * i] = r;
+            r = block_sum(ay[i], sh);
+            if (t == 0) partial[(size_t)blockIdx.x * MAXV + 2 * i + 1] = r;
+        }
+    }
+}
+
 // partial[b][0], [1] = Re, Im of sum conj(phi_k) psi_k
 __global__ void __launch_bounds__(RB) k_overlap(const double2* __restrict__ phi, const double2* __restrict__ psi,
                                                 uint64_t dim, double* __restrict__ partial)
@@ -97,6 +149,92 @@ __global__ void __launch_bounds__(RB) k_overlap(const double2* __restrict__ phi,
     if (threadIdx.x == 0) partial[(size_t)blockIdx.x * MAXV] = r;
     r = block_sum(si, sh);
     if (threadIdx.x == 0) partial[(size_t)blockIdx.x * MAXV + 1] = r;
+}
+
+// partial[b][0] = sum over i with bit j = 0 of w(i) Re( conj(c_{i xor m}) c_i ),  m = 2^j + 2^k:
+//   alpha = x: w = 1/2 (the pair i, i xor m contributes twice 1/4);  alpha = y: w = -2 sigma_j sigma_k;
+// alpha = z: partial[b][0] = sum_i sigma_j sigma_k |c_i|^2 over ALL i (npairs = dim).      <S^a_j S^a_k>, P:203 / A15
+__global__ void __launch_bounds__(RB) k_corr(const double2* __restrict__ psi, int alpha, int j, int k, uint64_t n,
+                                             double* __restrict__ partial)
+{
+    __shared__ double sh[RB / 32];
+    double acc = 0.0;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t bj = (uint64_t)1 << j, bk = (uint64_t)1 << k;
+    if (alpha == TS_Z) {
+        for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+            const double2 c = psi[i];
+            const double p = c.x * c.x + c.y * c.y;
+            acc += (((i & bj) != 0) == ((i & bk) != 0)) ? 0.25 * p : -0.25 * p;
+        }
+    } else {
+        const uint64_t lowmask = bj - 1;
+        for (uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
+            const uint64_t i = ((q & ~lowmask) << 1) | (q & lowmask);          // bit j = 0
+            const double2 c0 = psi[i], c1 = psi[i ^ (bj | bk)];
+            const double re = c1.x * c0.x + c1.y * c0.y;
+            if (alpha == TS_X) acc += 0.5 * re;
+            else acc += (i & bk) ? 0.5 * re : -0.5 * re;                      // -2 sigma_j sigma_k, sigma_j = -1/2
+        }
+    }
+    const double r = block_sum(acc, sh);
+    if (threadIdx.x == 0) partial[(size_t)blockIdx.x * MAXV] = r;
+}
+
+// partial[b][0] = sum_k E(k) |c_k|^2 with E(k) = sum_j sigma_j (h_j + sum_{m<j} Jeff_jm sigma_m) evaluated from the
+// definition (O(N^2) per amplitude): an observable, not on the time-step path.
+__global__ void __launch_bounds__(RB) k_energy_diag(const double2* __restrict__ psi, int N, uint64_t dim,
+                                                    const double* __restrict__ h, const double* __restrict__ Jeff,
+                                                    double* __restrict__ partial)
+{
+    __shared__ double sh[RB / 32];
+    __shared__ double shh[TS_MAX_N];
+    __shared__ double sJ[TS_MAX_N * TS_MAX_N];
+    for (int i = threadIdx.x; i < N; i += blockDim.x) shh[i] = h[i];
+    for (int i = threadIdx.x; i < N * N; i += blockDim.x) sJ[i] = Jeff[(i / N) * TS_MAX_N + (i % N)];
+    __syncthreads();
+    double acc = 0.0;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < dim; k += stride) {
+        double E = 0.0;
+        for (int j = 0; j < N; ++j) {
+            const double sj = (double)((k >> j) & 1) - 0.5;
+            double f = shh[j];
+            for (int m = 0; m < j; ++m) f += sJ[j * N + m] * ((double)((k >> m) & 1) - 0.5);
+            E += sj * f;
+        }
+        const double2 c = psi[k];
+        acc += E * (c.x * c.x + c.y * c.y);
+    }
+    const double r = block_sum(acc, sh);
+    if (threadIdx.x == 0) partial[(size_t)blockIdx.x * MAXV] = r;
+}
+
+// Eq. A.1: spin u up, the other N-1 spins in an equal-weight superposition with random phases
+//   phi_j = 2 pi (splitmix64(seed + (j + 1) * 0x9E3779B97F4A7C15) >> 11) 2^-53,  j = amplitude index with bit u removed
+// (a counter-based stream: phase j needs no state; SplitMix64 of Steele, Lea & Flood).
+__device__ __forceinline__ uint64_t splitmix64_mix(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+__global__ void k_fill_random_phase(double2* __restrict__ psi, uint64_t dim, int u, uint64_t seed, double amp)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t ub = (uint64_t)1 << u;
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < dim; k += stride) {
+        double2 v = make_double2(0.0, 0.0);
+        if (k & ub) {
+            const uint64_t j = ((k >> (u + 1)) << u) | (k & (ub - 1));
+            const double x = (double)(splitmix64_mix(seed + (j + 1) * 0x9E3779B97F4A7C15ull) >> 11) * 0x1.0p-53;
+            double sn, cs;
+            sincos(2.0 * 3.14159265358979323846 * x, &sn, &cs);
+            v = make_double2(amp * cs, amp * sn);
+        }
+        psi[k] = v;
+    }
 }
 
 // out[v] = sum_b partial[b][v], b ascending (fixed order -> deterministic)
@@ -244,4 +382,70 @@ cudaError_t ts_fill_basis(ts_ctx* c, uint64_t k)
     k_fill_basis<<<red_grid(dim), RB, 0, c->stream>>>(c->psi, dim, k);
     ts_prof_end(c);
     return cudaGetLastError();
+}
+
+cudaError_t ts_reduce_corr(ts_ctx* c, int alpha, int j, int k, double* out_host)
+{
+    if (alpha != TS_Z && j > k) { const int t = j; j = k; k = t; }      // the pair loop removes bit j: any order works, keep j < k
+    const uint64_t n = (alpha == TS_Z) ? (uint64_t)1 << c->N : (uint64_t)1 << (c->N - 1);
+    const int grid = red_grid(n);
+    cudaError_t e = ensure_scratch(c, (size_t)(grid + 1) * MAXV);
+    if (e != cudaSuccess) return e;
+    ts_prof_begin(c, TS_KC_REDUCE);
+    k_corr<<<grid, RB, 0, c->stream>>>(c->psi, alpha, j, k, n, c->d_red);
+    return finish(c, grid, 1, out_host);
+}
+
+cudaError_t ts_reduce_energy_diag(ts_ctx* c, int alpha, double* out_host)
+{
+    const uint64_t dim = (uint64_t)1 << c->N;
+    const int grid = red_grid(dim);
+    cudaError_t e = ensure_scratch(c, (size_t)(grid + 1) * MAXV);
+    if (e != cudaSuccess) return e;
+    ts_prof_begin(c, TS_KC_REDUCE);
+    k_energy_diag<<<grid, RB, 0, c->stream>>>(c->psi, c->N, dim, c->d_h + alpha * TS_MAX_N,
+                                               c->d_Jeff + (size_t)alpha * TS_MAX_N * TS_MAX_N, c->d_red);
+    return finish(c, grid, 1, out_host);
+}
+
+cudaError_t ts_fill_random_phase(ts_ctx* c, int up_spin, uint64_t seed)
+{
+    const uint64_t dim = (uint64_t)1 << c->N;
+    ts_prof_begin(c, TS_KC_SETUP);
+    k_fill_random_phase<<<red_grid(dim), RB, 0, c->stream>>>(c->psi, dim, up_spin, seed, 1.0 / sqrt(ldexp(1.0, c->N - 1)));
+    ts_prof_end(c);
+    return cudaGetLastError();
+}
+
+// <S^x_j> and <S^y_j> of ALL sites: one read-only pass per bit group of the plan (N = 30: 3 passes instead of 30).
+cudaError_t ts_reduce_expect_xy_all(ts_ctx* c, double* out_x /*[N] or NULL*/, double* out_y /*[N] or NULL*/)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute((const void*)k_pair_xy_group, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(sizeof(double2) << TS_TILE_LOG2));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
+    uint64_t g = ntiles < (uint64_t)(2 * c->num_sms) ? ntiles : (uint64_t)(2 * c->num_sms);
+    const int grid = (int)g;
+    cudaError_t e = ensure_scratch(c, (size_t)(grid + 1) * MAXV);
+    if (e != cudaSuccess) return e;
+    for (const TileGroup& tg : c->groups) {
+        const int f0 = tg.is_low ? 0 : tg.s;
+        const int nb = TS_TILE_LOG2 - f0;
+        ts_prof_begin(c, TS_KC_REDUCE);
+        k_pair_xy_group<<<grid, XG_T, sizeof(double2) << TS_TILE_LOG2, c->stream>>>(c->psi, ntiles, tg.s, tg.g0, f0, nb, c->d_red);
+        double v[2 * TS_TILE_LOG2];
+        e = finish(c, grid, 2 * nb, v);
+        if (e != cudaSuccess) return e;
+        for (int i = 0; i < nb; ++i) {
+            const int f = f0 + i;
+            const int spin = f < tg.s ? f : tg.g0 + (f - tg.s);
+            if (out_x) out_x[spin] = v[2 * i];
+            if (out_y) out_y[spin] = v[2 * i + 1];
+        }
+    }
+    return cudaSuccess;
 }

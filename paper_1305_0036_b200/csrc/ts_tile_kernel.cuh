@@ -1,5 +1,7 @@
-// ts_tile_kernel.cuh -- the tile-pass kernel template.  Included by the ts_tile_cfg*.cu translation
-// units (one per tile configuration, compiled in parallel) and by ts_tile.cu (launcher, phase tables).
+// ts_tile_kernel.cuh -- the tile-pass arithmetic and its first kernel, k_tile_pass: one CTA per tile,
+// loads and stores straight from registers.  The production kernels (ts_tile_v2.cuh) reuse the butterfly and
+// phase-table code below and differ in how tiles travel; k_tile_pass stays as the fallback for geometries they do not
+// take and as the A/B baseline.  Included by ts_tile_cfgG.cu, ts_tile_v2.cuh and ts_tile.cu.
 //
 // One launch = one HBM round trip of the whole state.  Each CTA (128 threads) owns one closed tile of 2^12
 // amplitudes (the set of states with the spins outside the tile fixed "is closed under the pairing operation
@@ -35,16 +37,6 @@
 #pragma once
 #include "ts_internal.h"
 
-// Tile configuration: which register bits are butterflied in layout 1 (BF1) and layout 2 (BF2; 0 = layout 2 unused),
-// and how many lane bits (group A only).  BF1 < 0: masks are run-time parameters (generic kernel).
-#define TS_CFG_GENERIC 0
-#define TS_CFG_A 1
-#define TS_CFG_H7 2
-#define TS_CFG_H8 3
-#define TS_CFG_H9 4
-#define TS_CFG_H10 5
-#define TS_CFG_COUNT 6
-
 struct TilePassParams {
     double2* psi;
     uint64_t tile_base;          // first tile of this launch (L2-blocked runs launch a window of tiles)
@@ -61,13 +53,8 @@ struct TilePassParams {
 
 typedef void (*tile_kernel_t)(const TilePassParams);
 
-// registry filled by the per-configuration translation units
+// registry filled by ts_tile_cfgG.cu
 void ts_tile_register_generic(tile_kernel_t (*tab)[5][5]);
-void ts_tile_register_A(tile_kernel_t (*tab)[5][5]);
-void ts_tile_register_H7(tile_kernel_t (*tab)[5][5]);
-void ts_tile_register_H8(tile_kernel_t (*tab)[5][5]);
-void ts_tile_register_H9(tile_kernel_t (*tab)[5][5]);
-void ts_tile_register_H10(tile_kernel_t (*tab)[5][5]);
 
 #ifdef __CUDACC__
 namespace tsk {
@@ -182,8 +169,7 @@ __device__ __forceinline__ void apply_diag(const TilePassParams& p, double2 base
 }
 
 // One tile: load (layout 1), sweep K1, diagonal, sweep K2, store in place.  CG bit 0: bypass L1 on the loads
-// (ld.global.cg; needed when another SM wrote the tile earlier in the SAME launch, see ts_tile_chunk.cuh); bit 1: keep
-// the stores in L2 (st.global.cg) instead of streaming them out (st.global.cs).
+// (ld.global.cg); bit 1: keep the stores in L2 (st.global.cg) instead of streaming them out (st.global.cs).
 template <int K1, int K2, int BF1, int BF2, int NSHFL, int CG>
 __device__ __forceinline__ void tile_body(const TilePassParams& p, const uint64_t tau, double2* sm)
 {
@@ -265,21 +251,6 @@ __global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __gri
     extern __shared__ double2 sm[];          // 4096 slots when layout 2 is used
     tile_body<K1, K2, BF1, BF2, NSHFL, 0>(p, p.tile_base + blockIdx.x, sm);
 }
-
-// The kernels a configuration needs: 4 fused transitions, 4 single sweeps, and "diagonal, then X^dag" (first pass).
-#define TS_TILE_REGISTER_CFG(NAME, BF1, BF2, NSHFL, MINB)                                                         \
-    void ts_tile_register_##NAME(tile_kernel_t (*tab)[5][5])                                                      \
-    {                                                                                                             \
-        (*tab)[SW_XDAG][SW_YDAG] = tsk::k_tile_pass<SW_XDAG, SW_YDAG, BF1, BF2, NSHFL, MINB>;                     \
-        (*tab)[SW_YDAG][SW_Y]    = tsk::k_tile_pass<SW_YDAG, SW_Y, BF1, BF2, NSHFL, MINB>;                        \
-        (*tab)[SW_Y][SW_X]       = tsk::k_tile_pass<SW_Y, SW_X, BF1, BF2, NSHFL, MINB>;                           \
-        (*tab)[SW_X][SW_XDAG]    = tsk::k_tile_pass<SW_X, SW_XDAG, BF1, BF2, NSHFL, MINB>;                        \
-        (*tab)[SW_YDAG][SW_NONE] = tsk::k_tile_pass<SW_YDAG, SW_NONE, BF1, BF2, NSHFL, MINB>;                     \
-        (*tab)[SW_Y][SW_NONE]    = tsk::k_tile_pass<SW_Y, SW_NONE, BF1, BF2, NSHFL, MINB>;                        \
-        (*tab)[SW_XDAG][SW_NONE] = tsk::k_tile_pass<SW_XDAG, SW_NONE, BF1, BF2, NSHFL, MINB>;                     \
-        (*tab)[SW_X][SW_NONE]    = tsk::k_tile_pass<SW_X, SW_NONE, BF1, BF2, NSHFL, MINB>;                        \
-        (*tab)[SW_NONE][SW_XDAG] = tsk::k_tile_pass<SW_NONE, SW_XDAG, BF1, BF2, NSHFL, MINB>;                     \
-    }
 
 } // namespace tsk
 #endif

@@ -1,0 +1,570 @@
+// ts_tile_v2.cuh -- the tile pass as a warp-specialised, TMA-in / TMA-out persistent kernel (
+// DESIGN.md 7.2).  Same mathematics as k_tile_pass (ts_tile_kernel.cuh): a closed tile of 2^12 amplitudes is
+// held in registers, 32 amplitudes per thread, and gets  [butterflies of sweep K1] . [diagonal D] . [butterflies of
+// sweep K2]  on the bits of its group before it is written back in place.  What differs is how the tile travels:
+//
+//   * one CTA per SM, 10 warps: 8 compute warps = two groups of 128 threads that take alternate tiles, one LOADER warp
+//     and one STORER warp (one elected lane each).  No compute thread ever forms a global address.
+//   * three 64-KiB tile buffers in shared memory.  The loader fills a buffer with two TMA tensor boxes of 32 KiB
+//     (cp.async.bulk.tensor, 128-byte swizzle, completion on the buffer's `full` mbarrier); a compute group works on it
+//     IN PLACE -- the register<->register layout exchanges of the butterfly network go through the tile's own buffer,
+//     every thread overwriting exactly the slots it read, so an exchange costs ONE group barrier -- and leaves the
+//     finished tile in the buffer; the storer writes it back with two TMA tensor stores and hands the buffer back to
+//     the loader when the store has read it.  Loads, stores and arithmetic of different tiles overlap without any
+//     thread waiting on a memory instruction of its own.
+//   * shared-memory slot of in-tile index f:  slot(f) = f ^ ((f >> 3) & 7)  -- exactly what TMA's SWIZZLE_128B writes
+//     for rows of 8 amplitudes (128 B).  All register layouts below keep one of {f0|f3}, {f1|f4}, {f2|f5} on each of
+//     the three low lane bits, which makes every 128-bit shared-memory access conflict-free under that swizzle.
+//
+// In-tile index f (12 bits): group A (spins 0..11): f = spin.  High group (s run bits, m = 12 - s group bits):
+// f < s <-> spin f, f >= s <-> spin g0 + f - s; the tile is 2^m rows of 2^s amplitudes at a stride of 2^g0.
+//
+// Register layouts (r = register index, 5 bits; t = thread index in the group, 7 bits; lists give the f bit of each
+// register / thread bit):
+//   A1: regs {3,4,5,10,11}  threads {0,1,2,8,9,6,7}        A2: regs {0,1,2,8,9}  threads {3,4,5,6,7,10,11}
+//   H1: regs {7,8,9,10,11}  threads {0,1,2,3,4,5,6}        H2: regs {3,4,5,6,7}  threads {0,1,2,8,9,10,11}
+// Group A butterflies all 12 bits: 5 in A1, 5 in A2 and f6, f7 (lane bits 3, 4 of A2) by warp shuffles; the diagonal is
+// applied in A2.  A high group butterflies f >= s: f7..11 in H1 and f_s..6 in H2 (m > 5 only; diagonal in H2, else H1).
+#pragma once
+#include <cuda.h>
+
+#include "ts_tile_kernel.cuh"
+
+#define TS_V2_THREADS 384                 // two compute warpgroups (8 warps) + one producer warpgroup (loader warp, storer warp, 2 idle)
+#define TS_V2_REGS_COMPUTE 232            // setmaxnreg: 256 x 232 + 128 x 40 = 64 512 <= 65 536 registers
+#define TS_V2_REGS_PRODUCER 40
+#define TS_V2_NBUF 3
+#define TS_V2_TILE_BYTES 65536
+#define TS_V2_OFF_TP (TS_V2_NBUF * TS_V2_TILE_BYTES)         // 3 x 512 B tile-phase records
+#define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3] mbarriers
+#define TS_V2_SMEM (TS_V2_OFF_BAR + 128)
+
+#define TS_V2_A1_R 0xBA543u
+#define TS_V2_A1_T 0x7698210u
+#define TS_V2_A2_R 0x98210u
+#define TS_V2_A2_T 0xBA76543u
+#define TS_V2_H1_R 0xBA987u
+#define TS_V2_H1_T 0x6543210u
+#define TS_V2_H2_R 0x76543u
+#define TS_V2_H2_T 0xBA98210u
+
+// One tile group as the kernel sees it.
+struct V2Geom {
+    int type;               // 0: group A (contiguous tile), 1: high group
+    int s, g0, m;           // high group: run bits, first spin, group bits (A: 12, 12, 0)
+    int nmid;               // g0 - s: tile-index bits below the group
+    int two_stage;          // high group with m > 5: layouts H1 and H2
+    unsigned mask1, mask2;  // butterflied register bits in H1 / H2
+};
+
+// Phase tables of the diagonal applied by a pass (see ts_tile_kernel.cuh for their meaning); tile_phase = NULL: none.
+struct V2Diag {
+    const double2* tile_phase;   // [ntiles][32]
+    const double2* TT;           // [128]
+    const double2* WT;           // [5][128]
+    double scale;                // exact power of two
+    double2 RR[32];
+};
+
+struct V2Pass {
+    V2Geom g;
+    V2Diag d;
+    uint64_t ntiles;
+};
+
+// L2-blocked triple launch: [high group, sweep KA] [group A: KA . D . KB] [high group, sweep KB] chunk by chunk.
+struct V2Chunk {
+    V2Geom gh, ga;
+    V2Diag d;
+    unsigned int* done;          // [2][nchunks] tiles finished (and globally visible) of phase 1 / phase 2 of a chunk
+    uint32_t nchunks, tiles_log2;
+};
+
+typedef void (*v2_kernel_t)(const V2Pass, const CUtensorMap);
+typedef void (*v2_chunk_kernel_t)(const V2Chunk, const CUtensorMap, const CUtensorMap);
+
+// tab[type][k1][k2]
+void ts_v2_register_A(v2_kernel_t (*tab)[5][5]);
+void ts_v2_register_Hf(v2_kernel_t (*tab)[5][5]);
+void ts_v2_register_Hs(v2_kernel_t (*tab)[5][5]);
+// tab[v]: v = 0: (Y^dag, Y), v = 1: (X, X^dag) -- the two kind pairs that meet at group A in the sweep order
+void ts_v2_register_chunk0(v2_chunk_kernel_t* tab);
+void ts_v2_register_chunk1(v2_chunk_kernel_t* tab);
+
+#ifdef __CUDACC__
+namespace tsk {
+
+// ------------------------------------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t v2_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void v2_mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void v2_mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void v2_mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void v2_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void v2_bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void v2_tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+                 "l"(tm), "r"(bar), "r"(c0), "r"(c1)
+                 : "memory");
+}
+__device__ __forceinline__ void v2_tma_load_4d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(dst),
+        "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+__device__ __forceinline__ void v2_tma_store_2d(const CUtensorMap* tm, uint32_t src, int c0, int c1)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%2, %3}], [%1];" ::"l"(tm), "r"(src), "r"(c0),
+                 "r"(c1)
+                 : "memory");
+}
+__device__ __forceinline__ void v2_tma_store_4d(const CUtensorMap* tm, uint32_t src, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(tm), "r"(src),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+                 : "memory");
+}
+__device__ __forceinline__ void v2_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void v2_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void v2_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void v2_fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void v2_fence_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void v2_group_sync(int grp)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(TS_TILE_THREADS) : "memory");
+}
+template <int R> __device__ __forceinline__ void v2_regs_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(R)); }
+template <int R> __device__ __forceinline__ void v2_regs_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R)); }
+__device__ __forceinline__ unsigned int v2_ld_acquire(const unsigned int* p)
+{
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------ register layouts
+// RP / TP: the f bit of register bit i / thread bit i, one nibble each.
+template <uint32_t RP, uint32_t TP>
+struct V2Layout {
+    // byte offset (within a tile buffer) of the slot of the thread part of f
+    static __device__ __forceinline__ uint32_t thread_off(int t)
+    {
+        uint32_t f = 0;
+#pragma unroll
+        for (int i = 0; i < 7; ++i) f |= (uint32_t)((t >> i) & 1) << ((TP >> (4 * i)) & 15u);
+        return (f ^ ((f >> 3) & 7u)) << 4;
+    }
+    static __host__ __device__ constexpr uint32_t reg_slot(int r)
+    {
+        uint32_t f = 0;
+        for (int i = 0; i < 5; ++i) f |= (uint32_t)((r >> i) & 1) << ((RP >> (4 * i)) & 15u);
+        return f ^ ((f >> 3) & 7u);
+    }
+    // slot(f_t | f_r) = slot(f_t) ^ slot(f_r) (the swizzle is linear over bits); only the three low slot bits mix
+    static __device__ __forceinline__ double2* ptr(unsigned char* buf, uint32_t toff, int r)
+    {
+        const uint32_t c = reg_slot(r);
+        return reinterpret_cast<double2*>(buf + ((toff ^ ((c & 7u) << 4)) + ((c & ~7u) << 4)));
+    }
+    static __device__ __forceinline__ void load(unsigned char* buf, uint32_t toff, double (&re)[32], double (&im)[32])
+    {
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            const double2 v = *ptr(buf, toff, r);
+            re[r] = v.x; im[r] = v.y;
+        }
+    }
+    static __device__ __forceinline__ void store(unsigned char* buf, uint32_t toff, const double (&re)[32], const double (&im)[32])
+    {
+#pragma unroll
+        for (int r = 0; r < 32; ++r) *ptr(buf, toff, r) = make_double2(re[r], im[r]);
+    }
+};
+
+// Per-thread phase factors from the tile-phase record `tp` (32 entries, in shared memory) and the thread tables.
+__device__ __forceinline__ void v2_thread_phase(const V2Diag& d, const double2* tp, const int t, double2& base, double2 (&w)[5])
+{
+    base = cmul(tp[0], __ldg(d.TT + t));
+    base = cmul(base, tp[1 + (t & 15)]);
+    base = cunit(cmul(base, tp[17 + (t >> 4)]));
+    base.x *= d.scale; base.y *= d.scale;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) w[k] = cunit(cmul(tp[25 + k], __ldg(d.WT + k * 128 + t)));
+}
+
+// c_r <- c_r * base * RR[r] * prod_i w_i^{r_i}   (depth-first product tree)
+__device__ __forceinline__ void v2_apply_diag(const V2Diag& d, const double2 base, const double2 (&w)[5], double (&re)[32],
+                                              double (&im)[32])
+{
+#pragma unroll
+    for (int b4 = 0; b4 < 2; ++b4) {
+        const double2 q4 = b4 ? cmul(base, w[4]) : base;
+#pragma unroll
+        for (int b3 = 0; b3 < 2; ++b3) {
+            const double2 q3 = b3 ? cmul(q4, w[3]) : q4;
+#pragma unroll
+            for (int b2 = 0; b2 < 2; ++b2) {
+                const double2 q2 = b2 ? cmul(q3, w[2]) : q3;
+#pragma unroll
+                for (int b1 = 0; b1 < 2; ++b1) {
+                    const double2 q1 = b1 ? cmul(q2, w[1]) : q2;
+#pragma unroll
+                    for (int b0 = 0; b0 < 2; ++b0) {
+                        const double2 q0 = b0 ? cmul(q1, w[0]) : q1;
+                        const int r = b0 | (b1 << 1) | (b2 << 2) | (b3 << 3) | (b4 << 4);
+                        const double2 ph = cmul(q0, d.RR[r]);
+                        const double2 c = cmul(make_double2(re[r], im[r]), ph);
+                        re[r] = c.x; im[r] = c.y;
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ tile bodies
+// The tile is in `buf` (landed by TMA); on return the finished tile is in `buf` again, in the same slots.
+// d = NULL or d->tile_phase = NULL: no diagonal.  tp: this tile's phase record.
+template <int K1, int K2>
+__device__ __forceinline__ void v2_body_A(unsigned char* buf, const V2Diag* d, const double2* tp, const int t, const int grp)
+{
+    using L1 = V2Layout<TS_V2_A1_R, TS_V2_A1_T>;
+    using L2 = V2Layout<TS_V2_A2_R, TS_V2_A2_T>;
+    const int lane = t & 31;
+    const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t);
+    double re[32], im[32];
+    if (K1 != SW_NONE) {
+        L1::load(buf, o1, re, im);
+        bfly_regs<K1, 31>(re, im, 0u);                 // f 3,4,5,10,11
+        L1::store(buf, o1, re, im);
+        v2_group_sync(grp);
+    }
+    L2::load(buf, o2, re, im);
+    if (K1 != SW_NONE) {
+        bfly_regs<K1, 31>(re, im, 0u);                 // f 0,1,2,8,9
+        bfly_lane<K1>(re, im, 3, lane);                // f 6
+        bfly_lane<K1>(re, im, 4, lane);                // f 7
+    }
+    if (d != nullptr && d->tile_phase != nullptr) {
+        double2 base, w[5];
+        v2_thread_phase(*d, tp, t, base, w);
+        v2_apply_diag(*d, base, w, re, im);
+    }
+    if (K2 != SW_NONE) {
+        bfly_lane<K2>(re, im, 4, lane);
+        bfly_lane<K2>(re, im, 3, lane);
+        bfly_regs<K2, 31>(re, im, 0u);
+        L2::store(buf, o2, re, im);
+        v2_group_sync(grp);
+        L1::load(buf, o1, re, im);
+        bfly_regs<K2, 31>(re, im, 0u);
+        L1::store(buf, o1, re, im);
+    } else {
+        L2::store(buf, o2, re, im);
+    }
+}
+
+template <int K1, int K2>
+__device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, const V2Diag* d, const double2* tp, const int t,
+                                          const int grp)
+{
+    using L1 = V2Layout<TS_V2_H1_R, TS_V2_H1_T>;
+    using L2 = V2Layout<TS_V2_H2_R, TS_V2_H2_T>;
+    const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t);
+    const bool two = (g.two_stage != 0);
+    double re[32], im[32];
+    L1::load(buf, o1, re, im);
+    bfly_regs<K1, -1>(re, im, g.mask1);
+    if (two) {
+        L1::store(buf, o1, re, im);
+        v2_group_sync(grp);
+        L2::load(buf, o2, re, im);
+        bfly_regs<K1, -1>(re, im, g.mask2);
+    }
+    if (d != nullptr && d->tile_phase != nullptr) {
+        double2 base, w[5];
+        v2_thread_phase(*d, tp, t, base, w);
+        v2_apply_diag(*d, base, w, re, im);
+    }
+    if (K2 != SW_NONE) {
+        if (two) {
+            bfly_regs<K2, -1>(re, im, g.mask2);
+            L2::store(buf, o2, re, im);
+            v2_group_sync(grp);
+            L1::load(buf, o1, re, im);
+        }
+        bfly_regs<K2, -1>(re, im, g.mask1);
+        L1::store(buf, o1, re, im);
+    } else {
+        if (two) L2::store(buf, o2, re, im);
+        else L1::store(buf, o1, re, im);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ TMA issue
+// Tensor maps (ts_tile.cu): group A: the state as [2^(N-3)] rows of 16 doubles, box {16, 256}; high group: the state as
+// [top][2^m rows][2^(g0-3) units][16 doubles], box {16, 2^(s-3), 2^(m-1), 1}.  Two boxes (f bit 11 = 0 / 1) per tile.
+__device__ __forceinline__ void v2_tile_coords(const V2Geom& g, const uint64_t tile, int& c1, int& c2lo, int& c2hi, int& c3)
+{
+    if (g.type == 0) {
+        c1 = (int)(tile << 9); c2lo = 0; c2hi = 256; c3 = 0;          // (2-D: row = c1 + c2)
+    } else {
+        const uint64_t mid = tile & (((uint64_t)1 << g.nmid) - 1);
+        c1 = (int)(mid << (g.s - 3));
+        c2lo = 0; c2hi = 1 << (g.m - 1);
+        c3 = (int)(tile >> g.nmid);
+    }
+}
+__device__ __forceinline__ void v2_issue_load(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t dst,
+                                              const uint32_t bar)
+{
+    int c1, c2lo, c2hi, c3;
+    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
+    if (g.type == 0) {
+        v2_tma_load_2d(dst, tm, bar, 0, c1 + c2lo);
+        v2_tma_load_2d(dst + 32768u, tm, bar, 0, c1 + c2hi);
+    } else {
+        v2_tma_load_4d(dst, tm, bar, 0, c1, c2lo, c3);
+        v2_tma_load_4d(dst + 32768u, tm, bar, 0, c1, c2hi, c3);
+    }
+}
+__device__ __forceinline__ void v2_issue_store(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src)
+{
+    int c1, c2lo, c2hi, c3;
+    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
+    if (g.type == 0) {
+        v2_tma_store_2d(tm, src, 0, c1 + c2lo);
+        v2_tma_store_2d(tm, src + 32768u, 0, c1 + c2hi);
+    } else {
+        v2_tma_store_4d(tm, src, 0, c1, c2lo, c3);
+        v2_tma_store_4d(tm, src + 32768u, 0, c1, c2hi, c3);
+    }
+}
+
+// Compute threads wait for job j's tile: buffer b = j % 3, use u = j / 3.  A parity wait only tells "the barrier's current
+// phase has parity p" (block) from "it has the other parity" (pass), so it is sound only while the barrier is known to be
+// in phase u or u + 1.  `full[b]` could still be in phase u - 1 if the other group's job j - 3 had not even landed; so
+// first wait until that job has been CONSUMED (done[b], phase u - 1: it cannot run ahead of phase u before this very
+// job arrives on it, and this group saw phase u - 2 complete when it finished job j - 6), which implies that full[b]
+// completed phase u - 1.  Then full[b] is in phase u or u + 1 and the wait below is exact.
+__device__ __forceinline__ void v2_wait_full(const uint32_t bar_full, const uint32_t bar_done, const uint32_t use)
+{
+    if (use > 0) v2_mbar_wait(bar_done, (use - 1) & 1u);
+    v2_mbar_wait(bar_full, use & 1u);
+}
+
+__device__ __forceinline__ void v2_init_barriers(const uint32_t sBar)
+{
+    for (int k = 0; k < TS_V2_NBUF; ++k) {
+        v2_mbar_init(sBar + 8 * k, 1);                                // full: the loader's expect_tx arrive
+        v2_mbar_init(sBar + 8 * (TS_V2_NBUF + k), TS_TILE_THREADS);   // done: every thread of the compute group
+        v2_mbar_init(sBar + 8 * (2 * TS_V2_NBUF + k), 1);             // free: the storer
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    v2_fence_async_smem();
+}
+
+// ------------------------------------------------------------------------------------------------ one tile pass
+// TYPE 0: group A, 1: high group.  CTA b runs tiles b, b + G, ...
+template <int TYPE, int K1, int K2>
+__global__ void __launch_bounds__(TS_V2_THREADS, 1)
+k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap tmap)
+{
+    extern __shared__ __align__(1024) unsigned char smraw[];
+    const uint32_t sBase = v2_smem_u32(smraw);
+    const uint32_t sBar = sBase + TS_V2_OFF_BAR;
+    const int warp = threadIdx.x >> 5;
+    const uint64_t G = gridDim.x;
+    const uint64_t n_cta = (p.ntiles > blockIdx.x) ? (p.ntiles - blockIdx.x + G - 1) / G : 0;
+    const bool has_diag = (p.d.tile_phase != nullptr);
+
+    if (threadIdx.x == 0) {
+        if (sBase & 1023u) __trap();                   // the 128-byte swizzle is a function of the shared address
+        v2_init_barriers(sBar);
+    }
+    __syncthreads();
+
+    if (warp >= 8) {                                   // ---- producer warpgroup: hands its registers to the compute warpgroups
+        v2_regs_dec<TS_V2_REGS_PRODUCER>();
+        if (warp == 8 && (threadIdx.x & 31) == 0) {    // ---- loader
+            for (uint64_t j = 0; j < n_cta; ++j) {
+                const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+                if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
+                const uint64_t tile = blockIdx.x + j * G;
+                const uint32_t bar = sBar + 8 * b;
+                v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (has_diag ? 512u : 0u));
+                if (has_diag) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, p.d.tile_phase + (tile << 5), 512u, bar);
+                v2_issue_load(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+            }
+        } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
+            for (uint64_t j = 0; j < n_cta; ++j) {
+                const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+                v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
+                v2_issue_store(p.g, &tmap, blockIdx.x + j * G, sBase + b * TS_V2_TILE_BYTES);
+                v2_store_commit();
+                v2_store_wait_read();
+                v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
+            }
+            v2_store_wait_all();
+        }
+    } else {                                           // ---- compute warpgroups
+        v2_regs_inc<TS_V2_REGS_COMPUTE>();
+        const int grp = warp >> 2;
+        const int t = threadIdx.x & (TS_TILE_THREADS - 1);
+        for (uint64_t j = grp; j < n_cta; j += 2) {
+            const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+            v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
+            unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
+            const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
+            if constexpr (TYPE == 0) v2_body_A<K1, K2>(buf, &p.d, tp, t, grp);
+            else v2_body_H<K1, K2>(buf, p.g, &p.d, tp, t, grp);
+            v2_fence_async_smem();                     // my shared-memory writes -> visible to the TMA store
+            v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ L2-blocked triple
+// Jobs n = 0 .. 3 * nchunks * T - 1 (T = tiles per chunk) in blocks of one (phase, chunk):
+//     P1(0) P1(1) P2(0) P2(1) P3(0) | P1(c) P3(c-1) P2(c), c = 2 .. nchunks-1 | P3(nchunks-1)
+// P1 = high group, sweep KA (from HBM);  P2 = group A, KA . D . KB (from L2);  P3 = high group, sweep KB (from L2, then
+// out to HBM).  A chunk is closed under all three (closed-set argument of P:141 applied to spins 0 .. C-1), so two
+// chunks (64 MiB) live in the 126 MB L2 at any time and the state makes ONE HBM round trip for three tile passes.
+// CTA b runs jobs b, b + G, ... ; a job of phase 2 / 3 may be LOADED once all T tiles of the previous phase of its chunk
+// are stored and visible: the loader polls done[phase - 1][chunk] (acquire) before it issues the TMA load, the storer
+// publishes a tile (release) once its TMA store has completed.  Only the loader ever waits on other CTAs, the compute
+// groups and the storer keep draining the jobs already loaded, and jobs are issued in increasing n on every CTA: the
+// smallest unfinished job never depends on an unfinished one, so the launch cannot deadlock as long as all CTAs are
+// resident (cooperative launch).
+template <int KA, int KB>
+__global__ void __launch_bounds__(TS_V2_THREADS, 1)
+k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmH)
+{
+    extern __shared__ __align__(1024) unsigned char smraw[];
+    const uint32_t sBase = v2_smem_u32(smraw);
+    const uint32_t sBar = sBase + TS_V2_OFF_BAR;
+    const int warp = threadIdx.x >> 5;
+    const uint32_t tl = q.tiles_log2, T = 1u << tl;
+    const uint32_t nblocks = 3u * q.nchunks;
+    const uint64_t total = (uint64_t)nblocks << tl;
+    const uint64_t G = gridDim.x;
+    const uint64_t n_cta = (total > blockIdx.x) ? (total - blockIdx.x + G - 1) / G : 0;
+    const bool has_diag = (q.d.tile_phase != nullptr);
+
+    auto job_of = [&](const uint64_t j, uint32_t& phase, uint32_t& c, uint64_t& tile) {
+        const uint64_t n = blockIdx.x + j * G;
+        const uint32_t B = (uint32_t)(n >> tl);
+        if (B == nblocks - 1) { phase = 2; c = q.nchunks - 1; }
+        else if (B < 5) { phase = (B < 2) ? 0u : (B < 4 ? 1u : 2u); c = (B == 1 || B == 3) ? 1u : 0u; }
+        else {
+            const uint32_t k = B - 5, r = k % 3;
+            c = 2 + k / 3;
+            if (r == 0) phase = 0; else if (r == 1) { phase = 2; c -= 1; } else phase = 1;
+        }
+        tile = ((uint64_t)c << tl) | (n & (T - 1));
+    };
+
+    if (threadIdx.x == 0) {
+        if (sBase & 1023u) __trap();
+        v2_init_barriers(sBar);
+    }
+    __syncthreads();
+
+    if (warp >= 8) {                                   // ---- producer warpgroup
+        v2_regs_dec<TS_V2_REGS_PRODUCER>();
+        if (warp == 8 && (threadIdx.x & 31) == 0) {    // ---- loader
+            uint32_t ok_key = 0xffffffffu;             // (phase, chunk) whose dependency was last seen satisfied
+            for (uint64_t j = 0; j < n_cta; ++j) {
+                const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+                uint32_t phase, c; uint64_t tile;
+                job_of(j, phase, c, tile);
+                if (phase != 0) {
+                    const uint32_t key = (phase << 28) | c;
+                    if (key != ok_key) {
+                        const unsigned int* dp = q.done + (size_t)(phase - 1) * q.nchunks + c;
+                        while (v2_ld_acquire(dp) < T) __nanosleep(64);
+                        ok_key = key;
+                    }
+                    v2_fence_async_all();              // the TMA engine reads what other SMs' TMA stores wrote
+                }
+                if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
+                const uint32_t bar = sBar + 8 * b;
+                const bool tpl = has_diag && phase == 1;
+                v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (tpl ? 512u : 0u));
+                if (tpl) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, q.d.tile_phase + (tile << 5), 512u, bar);
+                if (phase == 1) v2_issue_load(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+                else v2_issue_load(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+            }
+        } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
+            for (uint64_t j = 0; j < n_cta; ++j) {
+                const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+                uint32_t phase, c; uint64_t tile;
+                job_of(j, phase, c, tile);
+                v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
+                if (phase == 1) v2_issue_store(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES);
+                else v2_issue_store(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES);
+                v2_store_commit();
+                if (phase != 2) {
+                    v2_store_wait_all();               // the tile is in global memory (L2) ...
+                    v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
+                    v2_fence_async_all();
+                    __threadfence();                   // ... before it is published to the other CTAs' loaders
+                    atomicAdd(q.done + (size_t)phase * q.nchunks + c, 1u);
+                } else {
+                    v2_store_wait_read();
+                    v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
+                }
+            }
+            v2_store_wait_all();
+        }
+    } else {                                           // ---- compute warpgroups
+        v2_regs_inc<TS_V2_REGS_COMPUTE>();
+        const int grp = warp >> 2;
+        const int t = threadIdx.x & (TS_TILE_THREADS - 1);
+        for (uint64_t j = grp; j < n_cta; j += 2) {
+            const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+            uint32_t phase, c; uint64_t tile;
+            job_of(j, phase, c, tile);
+            v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
+            unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
+            const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
+            if (phase == 0) v2_body_H<KA, SW_NONE>(buf, q.gh, nullptr, tp, t, grp);
+            else if (phase == 1) v2_body_A<KA, KB>(buf, &q.d, tp, t, grp);
+            else v2_body_H<KB, SW_NONE>(buf, q.gh, nullptr, tp, t, grp);
+            v2_fence_async_smem();
+            v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
+        }
+    }
+}
+
+} // namespace tsk
+#endif

@@ -235,6 +235,15 @@ def config(which) -> Workload:
     raise KeyError(which)
 
 
+def config5_like(N: int) -> Workload:
+    """BASELINE config 5's recipe (4-row open XYZ lattice, fields from seed 7, checkerboard Neel state, tau = 0.01) on
+    a 4 x (N/4) lattice: the size at which that Hamiltonian family can meet the full oracle (reading A23)."""
+    assert N % 4 == 0 and N >= 8
+    cols = N // 4
+    return _grid_workload(f"config5_like_grid{N}", 4, cols, N, 7, tau=0.01, n_steps=10,
+                          state_kind="basis", basis_index=checkerboard_index(4, cols))
+
+
 def grid_like(N: int, seed: int, tau: float = 0.01, n_steps: int = 2, state_seed: Optional[int] = None,
               cols: Optional[int] = None) -> Workload:
     """Same recipe as configs 4/5/M on a ceil(N/cols) x cols open grid truncated to N sites."""

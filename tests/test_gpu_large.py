@@ -85,11 +85,17 @@ def expected_observables(w, subs):
     return exp, float(np.prod(norms))
 
 
-def check_clustered(B, N, n_clusters, n_steps, seed, n_windows=64, window=1 << 14, xy_sites=(0, 13)):
+def check_clustered(B, N, n_clusters, n_steps, seed, n_windows=64, window=1 << 14, xy_sites=(0, 13), options=(),
+                    expect_chunk=False):
     w = W.clustered(N, W.interleaved_clusters(N, n_clusters), seed=seed, tau=0.02, n_steps=n_steps)
     ts = B.TrotterSuzuki(N, w.h, w.J)
+    for key, value in options:
+        ts.set_option(key, value)
     upload_cluster_product(ts, w)
+    ts.reset_profile()
     ts.evolve(w.tau, n_steps, 4)
+    if expect_chunk:
+        assert ts.get_profile()["tile_chunk3"]["launches"] == 10 * n_steps
     subs = oracle_cluster_states(w, n_steps)
     rng = np.random.Generator(np.random.PCG64(seed + 1))
     dim = 1 << N
@@ -122,8 +128,8 @@ def test_cluster_factorisation_N27(B):
 
 def test_cluster_factorisation_N30_bench_plan(B):
     """The metric size in the launch configuration bench.py times (default plan)."""
-    plan = check_clustered(B, 30, 3, 1, seed=30)
-    assert "A[spins 0..11]" in plan and "3 group" in plan
+    plan = check_clustered(B, 30, 3, 1, seed=30, expect_chunk=True)
+    assert "A[spins 0..11]" in plan and "3 group" in plan and "L2-blocked" in plan
 
 
 def test_cluster_factorisation_N32_in_place(B):
@@ -180,11 +186,19 @@ def test_config5_grid32_properties(B):
     ts.close()
 
 
-@pytest.mark.parametrize("pipe,chunk3", [(0, 0), (2, 0), (1, 1)])
-def test_kernel_variants_N26(B, pipe, chunk3, monkeypatch):
-    """The execution switches read at ts_create: first kernel only (TS_PIPE=0), pipelined kernel for
-    every tile pass (TS_PIPE=2), ticket-scheduled L2-blocked triple launch (TS_CHUNK3=1).  Same gate as the default
-    path, which the other tests of this file run (pipelined fused passes + pipelined triple launch at N = 30)."""
-    monkeypatch.setenv("TS_PIPE", str(pipe))
-    monkeypatch.setenv("TS_CHUNK3", str(chunk3))
-    check_clustered(B, 26, 3, 1, seed=2600 + 10 * pipe + chunk3, n_windows=32)
+@pytest.mark.parametrize("kernel,chunk", [(0, 0), (1, 0), (1, 1)])
+def test_kernel_variants_N26(B, kernel, chunk):
+    """The execution options (ts_set_option): one-CTA-per-tile kernels only, v2 kernels with every pass its
+    own launch, v2 with the L2-blocked triple launch (the default, which the other tests of this file run)."""
+    check_clustered(B, 26, 3, 1, seed=2600 + 10 * kernel + chunk, n_windows=32,
+                    options=((B.OPT_KERNEL, kernel), (B.OPT_CHUNK, chunk)))
+
+
+def test_cluster_factorisation_N30_repeated_bench_plan(B):
+    """The benchmark's launch configuration at its size, over and over in one process: different seeds, 4 steps each
+    (40 triple launches + 40 fused top-group launches per repeat), the gate asserted every time.  The inter-CTA
+    hand-over of the triple launch is the one place of the path where a race could hide; compute-sanitizer is not
+    available on this pool, so repetition is the tool."""
+    for rep in range(6):
+        plan = check_clustered(B, 30, 3, 4, seed=3000 + rep, n_windows=24, expect_chunk=True)
+        assert "L2-blocked" in plan
