@@ -13,8 +13,8 @@
 namespace {
 
 tile_kernel_t g_tab[5][5];                 // k_tile_pass, run-time butterfly masks
-v2_kernel_t g_v2[2][5][5];                 // [type][k1][k2]
-v2_chunk_kernel_t g_v2_chunk[2];           // (Y^dag, Y), (X, X^dag)
+v2_kernel_t g_v2[3][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits
+v2_chunk_kernel_t g_v2_chunk[2][2];        // [9-bit high group][(Y^dag, Y), (X, X^dag)]
 PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
 std::once_flag g_once;
 cudaError_t g_init_status = cudaSuccess;
@@ -32,6 +32,7 @@ inline int n_bfly(const TileGroup& g) { return g.is_low ? TS_TILE_LOG2 : TS_TILE
 inline bool two_stage(const TileGroup& g) { return n_bfly(g) > 5; }
 inline bool v2_geometry_ok(const TileGroup& g) { return g.is_low || (g.s >= 3 && g.s <= 11); }
 inline int nib(uint32_t pack, int i) { return (int)((pack >> (4 * i)) & 15u); }
+inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : 1); }     // kernel table index
 
 // layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2, H2 or H1).
 PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
@@ -174,23 +175,28 @@ void init_once()
     ts_v2_register_A(&g_v2[0]);
     ts_v2_register_Hf(&g_v2[1]);
     ts_v2_register_Hs(&g_v2[1]);
+    ts_v2_register_H9f(&g_v2[2]);
+    ts_v2_register_H9s(&g_v2[2]);
     memset(g_v2_chunk, 0, sizeof(g_v2_chunk));
     ts_v2_register_chunk0(g_v2_chunk);
     ts_v2_register_chunk1(g_v2_chunk);
+    ts_v2_register_chunk0_h9(g_v2_chunk);
+    ts_v2_register_chunk1_h9(g_v2_chunk);
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
     if (e == cudaSuccess && (qr != cudaDriverEntryPointSuccess || !fn)) e = cudaErrorNotSupported;
     if (e != cudaSuccess) { g_init_status = e; return; }
     g_encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
-    for (int ty = 0; ty < 2 && e == cudaSuccess; ++ty)
+    for (int ty = 0; ty < 3 && e == cudaSuccess; ++ty)
         for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
             for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
                 if (g_v2[ty][k1][k2])
                     e = cudaFuncSetAttribute((const void*)g_v2[ty][k1][k2], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
-    for (int v = 0; v < 2 && e == cudaSuccess; ++v)
-        if (g_v2_chunk[v])
-            e = cudaFuncSetAttribute((const void*)g_v2_chunk[v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
+    for (int hm = 0; hm < 2 && e == cudaSuccess; ++hm)
+        for (int v = 0; v < 2 && e == cudaSuccess; ++v)
+            if (g_v2_chunk[hm][v])
+                e = cudaFuncSetAttribute((const void*)g_v2_chunk[hm][v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
     for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
         for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
             if (g_tab[k1][k2])
@@ -231,23 +237,18 @@ void fill_v2_geom(const TileGroup& g, V2Geom* q)
     q->two_stage = (!g.is_low && q->m > 5) ? 1 : 0;
     q->mask1 = 0u; q->mask2 = 0u;
     if (!g.is_low) {
-        for (int i = 0; i < 5; ++i) if (nib(TS_V2_H1_R, i) >= g.s) q->mask1 |= 1u << i;
-        // H2 register bit 4 (f 7) is a filler: f 7 was butterflied in H1
-        for (int i = 0; i < 4; ++i) if (nib(TS_V2_H2_R, i) >= g.s) q->mask2 |= 1u << i;
+        q->mask1 = tsk::v2_h_mask1(q->m);
+        q->mask2 = tsk::v2_h_mask2(q->m);     // H2 register bit 4 (f 7) is a filler: f 7 was butterflied in H1
     }
 }
 
 void fill_v2_diag(const DiagTables* tb, V2Diag* d)
 {
-    d->tile_phase = nullptr; d->TT = nullptr; d->WT = nullptr; d->scale = 1.0;
+    d->tile_phase = nullptr; d->tables = nullptr; d->scale = 1.0;
     if (tb) {
         d->tile_phase = tb->d_tile_phase;
-        d->TT = tb->d_thread;
-        d->WT = tb->d_thread + 128;
+        d->tables = tb->d_thread;            // TT[128], WT[5][128], RR[32]
         d->scale = ldexp(1.0, tb->scale_pow);
-        memcpy(d->RR, tb->RR, sizeof(d->RR));
-    } else {
-        for (int r = 0; r < 32; ++r) d->RR[r] = make_double2(1.0, 0.0);
     }
 }
 
@@ -330,7 +331,7 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, int layout
     DiagTables* tb = new DiagTables();
     tb->alpha = d.alpha; tb->scale_pow = d.scale_pow; tb->group = group; tb->layout = layout; tb->t = d.t;
     tb->d_thread = nullptr; tb->d_tile_phase = nullptr;
-    cudaError_t e = cudaMalloc(&tb->d_thread, sizeof(double2) * 6 * 128);
+    cudaError_t e = cudaMalloc(&tb->d_thread, sizeof(double2) * (6 * 128 + 32));     // TT, WT[5], RR
     if (e == cudaSuccess) e = cudaMalloc(&tb->d_tile_phase, sizeof(double2) * 32 * ntiles);
     if (e != cudaSuccess) {
         if (tb->d_thread) cudaFree(tb->d_thread);
@@ -338,6 +339,8 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, int layout
         return e;
     }
     build_RR(c, q, d.alpha, tb->RR);
+    e = cudaMemcpyAsync(tb->d_thread + 6 * 128, tb->RR, sizeof(tb->RR), cudaMemcpyHostToDevice, c->stream);   // (tb is heap-allocated and lives as long as the cache entry)
+    if (e != cudaSuccess) { cudaFree(tb->d_thread); cudaFree(tb->d_tile_phase); delete tb; return e; }
     const double* dh = c->d_h + d.alpha * TS_MAX_N;
     const double* dJ = c->d_Jeff + (size_t)d.alpha * TS_MAX_N * TS_MAX_N;
     ts_prof_begin(c, TS_KC_SETUP);
@@ -356,7 +359,7 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
 {
     const TileGroup& g = c->groups[group];
     if (c->opt_kernel == 0 || !v2_geometry_ok(g)) return 0;
-    return g_v2[g.is_low ? 0 : 1][kind1][kind2] ? 1 : 0;
+    return g_v2[v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
 cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int kind2)
@@ -381,7 +384,7 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
         const uint64_t cap = (c->opt_max_ctas > 0 && c->opt_max_ctas < c->num_sms) ? (uint64_t)c->opt_max_ctas : (uint64_t)c->num_sms;
         const uint64_t grid = ntiles < cap ? ntiles : cap;
         ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
-        g_v2[g.is_low ? 0 : 1][kind1][kind2]<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
+        g_v2[v2_type(g)][kind1][kind2]<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
         ts_prof_end(c);
         return cudaGetLastError();
     }
@@ -405,7 +408,7 @@ bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
     if (C >= c->N || C > c->opt_chunk_max_log2) return false;          // at least two chunks, each small enough for L2
     const int v = (ka == SW_YDAG && kb == SW_Y) ? 0 : (ka == SW_X && kb == SW_XDAG) ? 1 : -1;
-    return v >= 0 && g_v2_chunk[v] != nullptr;
+    return v >= 0 && g_v2_chunk[g.s == 3 ? 1 : 0][v] != nullptr;
 }
 
 cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int kb)
@@ -448,7 +451,7 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
     ts_prof_begin(c, TS_KC_TILE_CHUNK, 3.0);
     // cooperative launch: the loaders wait on other CTAs' progress, so all CTAs must be resident (else: error, not a hang)
     void* args[3] = {(void*)&q, (void*)&tmA, (void*)&tmH};
-    e = cudaLaunchCooperativeKernel((const void*)g_v2_chunk[v], dim3((unsigned)grid), dim3(TS_V2_THREADS), args, TS_V2_SMEM, c->stream);
+    e = cudaLaunchCooperativeKernel((const void*)g_v2_chunk[g.s == 3 ? 1 : 0][v], dim3((unsigned)grid), dim3(TS_V2_THREADS), args, TS_V2_SMEM, c->stream);
     ts_prof_end(c);
     return e;
 }

@@ -36,8 +36,10 @@
 #define TS_V2_NBUF 3
 #define TS_V2_TILE_BYTES 65536
 #define TS_V2_OFF_TP (TS_V2_NBUF * TS_V2_TILE_BYTES)         // 3 x 512 B tile-phase records
-#define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3] mbarriers
-#define TS_V2_SMEM (TS_V2_OFF_BAR + 128)
+#define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3], tab mbarriers
+#define TS_V2_OFF_TAB (TS_V2_OFF_BAR + 128)                  // per-launch phase tables: TT[128], WT[5][128], RR[32]
+#define TS_V2_TAB_BYTES (800 * 16)
+#define TS_V2_SMEM (TS_V2_OFF_TAB + TS_V2_TAB_BYTES)
 
 #define TS_V2_A1_R 0xBA543u
 #define TS_V2_A1_T 0x7698210u
@@ -59,11 +61,9 @@ struct V2Geom {
 
 // Phase tables of the diagonal applied by a pass (see ts_tile_kernel.cuh for their meaning); tile_phase = NULL: none.
 struct V2Diag {
-    const double2* tile_phase;   // [ntiles][32]
-    const double2* TT;           // [128]
-    const double2* WT;           // [5][128]
+    const double2* tile_phase;   // [ntiles][32]: one 512-byte record per tile, loaded with the tile
+    const double2* tables;       // TT[128], WT[5][128], RR[32] (800 entries): copied to shared memory once per launch
     double scale;                // exact power of two
-    double2 RR[32];
 };
 
 struct V2Pass {
@@ -83,13 +83,18 @@ struct V2Chunk {
 typedef void (*v2_kernel_t)(const V2Pass, const CUtensorMap);
 typedef void (*v2_chunk_kernel_t)(const V2Chunk, const CUtensorMap, const CUtensorMap);
 
-// tab[type][k1][k2]
+// tab[type][k1][k2]; type 0: group A, 1: high group (run-time masks), 2: high group with 9 group bits
 void ts_v2_register_A(v2_kernel_t (*tab)[5][5]);
 void ts_v2_register_Hf(v2_kernel_t (*tab)[5][5]);
 void ts_v2_register_Hs(v2_kernel_t (*tab)[5][5]);
-// tab[v]: v = 0: (Y^dag, Y), v = 1: (X, X^dag) -- the two kind pairs that meet at group A in the sweep order
-void ts_v2_register_chunk0(v2_chunk_kernel_t* tab);
-void ts_v2_register_chunk1(v2_chunk_kernel_t* tab);
+void ts_v2_register_H9f(v2_kernel_t (*tab)[5][5]);
+void ts_v2_register_H9s(v2_kernel_t (*tab)[5][5]);
+// tab[hm][v]: hm = 0: any high group, 1: 9 group bits;  v = 0: (Y^dag, Y), v = 1: (X, X^dag) -- the two kind pairs that
+// meet at group A in the sweep order
+void ts_v2_register_chunk0(v2_chunk_kernel_t (*tab)[2]);
+void ts_v2_register_chunk1(v2_chunk_kernel_t (*tab)[2]);
+void ts_v2_register_chunk0_h9(v2_chunk_kernel_t (*tab)[2]);
+void ts_v2_register_chunk1_h9(v2_chunk_kernel_t (*tab)[2]);
 
 #ifdef __CUDACC__
 namespace tsk {
@@ -210,19 +215,21 @@ struct V2Layout {
     }
 };
 
-// Per-thread phase factors from the tile-phase record `tp` (32 entries, in shared memory) and the thread tables.
-__device__ __forceinline__ void v2_thread_phase(const V2Diag& d, const double2* tp, const int t, double2& base, double2 (&w)[5])
+// Per-thread phase factors from the tile-phase record `tp` (32 entries) and the thread tables `tab` (TT, WT), both in
+// shared memory.
+__device__ __forceinline__ void v2_thread_phase(const double scale, const double2* tp, const double2* tab, const int t, double2& base,
+                                                double2 (&w)[5])
 {
-    base = cmul(tp[0], __ldg(d.TT + t));
+    base = cmul(tp[0], tab[t]);
     base = cmul(base, tp[1 + (t & 15)]);
     base = cunit(cmul(base, tp[17 + (t >> 4)]));
-    base.x *= d.scale; base.y *= d.scale;
+    base.x *= scale; base.y *= scale;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) w[k] = cunit(cmul(tp[25 + k], __ldg(d.WT + k * 128 + t)));
+    for (int k = 0; k < 5; ++k) w[k] = cunit(cmul(tp[25 + k], tab[128 + k * 128 + t]));
 }
 
-// c_r <- c_r * base * RR[r] * prod_i w_i^{r_i}   (depth-first product tree)
-__device__ __forceinline__ void v2_apply_diag(const V2Diag& d, const double2 base, const double2 (&w)[5], double (&re)[32],
+// c_r <- c_r * base * RR[r] * prod_i w_i^{r_i}   (depth-first product tree; RR = tab + 768, broadcast reads)
+__device__ __forceinline__ void v2_apply_diag(const double2* RR, const double2 base, const double2 (&w)[5], double (&re)[32],
                                               double (&im)[32])
 {
 #pragma unroll
@@ -241,7 +248,7 @@ __device__ __forceinline__ void v2_apply_diag(const V2Diag& d, const double2 bas
                     for (int b0 = 0; b0 < 2; ++b0) {
                         const double2 q0 = b0 ? cmul(q1, w[0]) : q1;
                         const int r = b0 | (b1 << 1) | (b2 << 2) | (b3 << 3) | (b4 << 4);
-                        const double2 ph = cmul(q0, d.RR[r]);
+                        const double2 ph = cmul(q0, RR[r]);
                         const double2 c = cmul(make_double2(re[r], im[r]), ph);
                         re[r] = c.x; im[r] = c.y;
                     }
@@ -253,9 +260,10 @@ __device__ __forceinline__ void v2_apply_diag(const V2Diag& d, const double2 bas
 
 // ------------------------------------------------------------------------------------------------ tile bodies
 // The tile is in `buf` (landed by TMA); on return the finished tile is in `buf` again, in the same slots.
-// d = NULL or d->tile_phase = NULL: no diagonal.  tp: this tile's phase record.
+// diag: apply the diagonal; tp: this tile's phase record; tab: the launch's thread tables (both in shared memory).
 template <int K1, int K2>
-__device__ __forceinline__ void v2_body_A(unsigned char* buf, const V2Diag* d, const double2* tp, const int t, const int grp)
+__device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, const double scale, const double2* tp,
+                                          const double2* tab, const int t, const int grp)
 {
     using L1 = V2Layout<TS_V2_A1_R, TS_V2_A1_T>;
     using L2 = V2Layout<TS_V2_A2_R, TS_V2_A2_T>;
@@ -274,10 +282,10 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const V2Diag* d, c
         bfly_lane<K1>(re, im, 3, lane);                // f 6
         bfly_lane<K1>(re, im, 4, lane);                // f 7
     }
-    if (d != nullptr && d->tile_phase != nullptr) {
+    if (diag) {
         double2 base, w[5];
-        v2_thread_phase(*d, tp, t, base, w);
-        v2_apply_diag(*d, base, w, re, im);
+        v2_thread_phase(scale, tp, tab, t, base, w);
+        v2_apply_diag(tab + 768, base, w, re, im);
     }
     if (K2 != SW_NONE) {
         bfly_lane<K2>(re, im, 4, lane);
@@ -293,36 +301,46 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const V2Diag* d, c
     }
 }
 
-template <int K1, int K2>
-__device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, const V2Diag* d, const double2* tp, const int t,
-                                          const int grp)
+// Butterflied register bits of a high group with m group bits (s = 12 - m run bits): H1 register bit i <-> f 7 + i,
+// H2 register bit i <-> f 3 + i for i < 4 (bit 4 = f 7 is a filler, done in H1).
+__host__ __device__ constexpr unsigned v2_h_mask1(int m) { unsigned k = 0; for (int i = 0; i < 5; ++i) if (7 + i >= 12 - m) k |= 1u << i; return k; }
+__host__ __device__ constexpr unsigned v2_h_mask2(int m) { unsigned k = 0; for (int i = 0; i < 4; ++i) if (3 + i >= 12 - m) k |= 1u << i; return k; }
+
+// M > 0: the number of group bits is a compile-time constant (masks folded: no run-time branches around the butterfly
+// levels); M = -1: taken from g at run time.
+template <int K1, int K2, int M>
+__device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, const bool diag, const double scale, const double2* tp,
+                                          const double2* tab, const int t, const int grp)
 {
     using L1 = V2Layout<TS_V2_H1_R, TS_V2_H1_T>;
     using L2 = V2Layout<TS_V2_H2_R, TS_V2_H2_T>;
+    constexpr bool CT = (M > 0);
+    constexpr int MK1 = CT ? (int)v2_h_mask1(M > 0 ? M : 1) : -1;
+    constexpr int MK2 = CT ? (int)v2_h_mask2(M > 0 ? M : 1) : -1;
     const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t);
-    const bool two = (g.two_stage != 0);
+    const bool two = CT ? (M > 5) : (g.two_stage != 0);
     double re[32], im[32];
     L1::load(buf, o1, re, im);
-    bfly_regs<K1, -1>(re, im, g.mask1);
+    bfly_regs<K1, MK1>(re, im, g.mask1);
     if (two) {
         L1::store(buf, o1, re, im);
         v2_group_sync(grp);
         L2::load(buf, o2, re, im);
-        bfly_regs<K1, -1>(re, im, g.mask2);
+        bfly_regs<K1, MK2>(re, im, g.mask2);
     }
-    if (d != nullptr && d->tile_phase != nullptr) {
+    if (diag) {
         double2 base, w[5];
-        v2_thread_phase(*d, tp, t, base, w);
-        v2_apply_diag(*d, base, w, re, im);
+        v2_thread_phase(scale, tp, tab, t, base, w);
+        v2_apply_diag(tab + 768, base, w, re, im);
     }
     if (K2 != SW_NONE) {
         if (two) {
-            bfly_regs<K2, -1>(re, im, g.mask2);
+            bfly_regs<K2, MK2>(re, im, g.mask2);
             L2::store(buf, o2, re, im);
             v2_group_sync(grp);
             L1::load(buf, o1, re, im);
         }
-        bfly_regs<K2, -1>(re, im, g.mask1);
+        bfly_regs<K2, MK1>(re, im, g.mask1);
         L1::store(buf, o1, re, im);
     } else {
         if (two) L2::store(buf, o2, re, im);
@@ -389,12 +407,13 @@ __device__ __forceinline__ void v2_init_barriers(const uint32_t sBar)
         v2_mbar_init(sBar + 8 * (TS_V2_NBUF + k), TS_TILE_THREADS);   // done: every thread of the compute group
         v2_mbar_init(sBar + 8 * (2 * TS_V2_NBUF + k), 1);             // free: the storer
     }
+    v2_mbar_init(sBar + 8 * 3 * TS_V2_NBUF, 1);                       // tab: the launch's thread tables have landed
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     v2_fence_async_smem();
 }
 
 // ------------------------------------------------------------------------------------------------ one tile pass
-// TYPE 0: group A, 1: high group.  CTA b runs tiles b, b + G, ...
+// TYPE 0: group A, 1: high group (any m), 2: high group with m = 9 (masks folded).  CTA b runs tiles b, b + G, ...
 template <int TYPE, int K1, int K2>
 __global__ void __launch_bounds__(TS_V2_THREADS, 1)
 k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap tmap)
@@ -416,6 +435,10 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
     if (warp >= 8) {                                   // ---- producer warpgroup: hands its registers to the compute warpgroups
         v2_regs_dec<TS_V2_REGS_PRODUCER>();
         if (warp == 8 && (threadIdx.x & 31) == 0) {    // ---- loader
+            if (has_diag) {
+                v2_mbar_expect_tx(sBar + 8 * 3 * TS_V2_NBUF, TS_V2_TAB_BYTES);
+                v2_bulk_load(sBase + TS_V2_OFF_TAB, p.d.tables, TS_V2_TAB_BYTES, sBar + 8 * 3 * TS_V2_NBUF);
+            }
             for (uint64_t j = 0; j < n_cta; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
                 if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
@@ -440,13 +463,17 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
         v2_regs_inc<TS_V2_REGS_COMPUTE>();
         const int grp = warp >> 2;
         const int t = threadIdx.x & (TS_TILE_THREADS - 1);
+        const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
+        const double scale = p.d.scale;
+        if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
         for (uint64_t j = grp; j < n_cta; j += 2) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
             v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
             unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
             const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
-            if constexpr (TYPE == 0) v2_body_A<K1, K2>(buf, &p.d, tp, t, grp);
-            else v2_body_H<K1, K2>(buf, p.g, &p.d, tp, t, grp);
+            if constexpr (TYPE == 0) v2_body_A<K1, K2>(buf, has_diag, scale, tp, tab, t, grp);
+            else if constexpr (TYPE == 2) v2_body_H<K1, K2, 9>(buf, p.g, has_diag, scale, tp, tab, t, grp);
+            else v2_body_H<K1, K2, -1>(buf, p.g, has_diag, scale, tp, tab, t, grp);
             v2_fence_async_smem();                     // my shared-memory writes -> visible to the TMA store
             v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
         }
@@ -465,7 +492,7 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
 // groups and the storer keep draining the jobs already loaded, and jobs are issued in increasing n on every CTA: the
 // smallest unfinished job never depends on an unfinished one, so the launch cannot deadlock as long as all CTAs are
 // resident (cooperative launch).
-template <int KA, int KB>
+template <int KA, int KB, int HM>
 __global__ void __launch_bounds__(TS_V2_THREADS, 1)
 k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmH)
 {
@@ -502,6 +529,10 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
     if (warp >= 8) {                                   // ---- producer warpgroup
         v2_regs_dec<TS_V2_REGS_PRODUCER>();
         if (warp == 8 && (threadIdx.x & 31) == 0) {    // ---- loader
+            if (has_diag) {
+                v2_mbar_expect_tx(sBar + 8 * 3 * TS_V2_NBUF, TS_V2_TAB_BYTES);
+                v2_bulk_load(sBase + TS_V2_OFF_TAB, q.d.tables, TS_V2_TAB_BYTES, sBar + 8 * 3 * TS_V2_NBUF);
+            }
             uint32_t ok_key = 0xffffffffu;             // (phase, chunk) whose dependency was last seen satisfied
             for (uint64_t j = 0; j < n_cta; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
@@ -550,6 +581,9 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
         v2_regs_inc<TS_V2_REGS_COMPUTE>();
         const int grp = warp >> 2;
         const int t = threadIdx.x & (TS_TILE_THREADS - 1);
+        const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
+        const double scale = q.d.scale;
+        if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
         for (uint64_t j = grp; j < n_cta; j += 2) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
             uint32_t phase, c; uint64_t tile;
@@ -557,9 +591,9 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
             v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
             unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
             const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
-            if (phase == 0) v2_body_H<KA, SW_NONE>(buf, q.gh, nullptr, tp, t, grp);
-            else if (phase == 1) v2_body_A<KA, KB>(buf, &q.d, tp, t, grp);
-            else v2_body_H<KB, SW_NONE>(buf, q.gh, nullptr, tp, t, grp);
+            if (phase == 0) v2_body_H<KA, SW_NONE, HM>(buf, q.gh, false, 1.0, tp, tab, t, grp);
+            else if (phase == 1) v2_body_A<KA, KB>(buf, has_diag, scale, tp, tab, t, grp);
+            else v2_body_H<KB, SW_NONE, HM>(buf, q.gh, false, 1.0, tp, tab, t, grp);
             v2_fence_async_smem();
             v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
         }

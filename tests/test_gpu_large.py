@@ -95,7 +95,7 @@ def check_clustered(B, N, n_clusters, n_steps, seed, n_windows=64, window=1 << 1
     ts.reset_profile()
     ts.evolve(w.tau, n_steps, 4)
     if expect_chunk:
-        assert ts.get_profile()["tile_chunk3"]["launches"] == 10 * n_steps
+        assert ts.get_profile()["tile_chunk3"]["launches"] == 10 * n_steps - 1
     subs = oracle_cluster_states(w, n_steps)
     rng = np.random.Generator(np.random.PCG64(seed + 1))
     dim = 1 << N

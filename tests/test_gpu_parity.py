@@ -57,13 +57,15 @@ def check_obs(ts, psi_ref, N):
     assert abs(ts.norm2() - O.norm2(psi_ref, N)) <= OBS_TOL
 
 
-# --------------------------------------------------------------------------------------------- naive path (N < 12)
+# --------------------------------------------------------------------------------------------- small N (N < 12)
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 8, 11])
 @pytest.mark.parametrize("order", [2, 4])
-def test_naive_generic(B, N, order):
+@pytest.mark.parametrize("plan", ["auto", "naive"])
+def test_small_N_generic(B, N, order, plan):
+    """plan = auto: the single-CTA path (ts_small.cu); plan = naive: the paper's launch-per-spin scheme (ts_naive.cu)."""
     w = W.generic(N, seed=100 + N, tau=0.02, n_steps=3, order=order, symmetric_fill=(N % 2 == 1))
-    ts = run_gpu(B, w)
-    assert "naive" in ts.describe_plan()
+    ts = run_gpu(B, w, plan=(B.PLAN_NAIVE, 0, 0) if plan == "naive" else None)
+    assert ("naive" if plan == "naive" else "small") in ts.describe_plan()
     ref = run_oracle(w)
     check_amps(ts.get_state(), ref)
     check_obs(ts, ref, N)

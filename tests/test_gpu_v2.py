@@ -91,7 +91,7 @@ def test_default_plan_N24_triple_launch_three_steps(B):
     ts.evolve(w.tau, 3, 4)
     prof = ts.get_profile()
     assert "L2-blocked" in ts.describe_plan()
-    assert prof["tile_chunk3"]["launches"] == 3 * 10, prof        # 10 per 4th-order step
+    assert prof["tile_chunk3"]["launches"] == 3 * 10 - 1, prof    # one per sweep pair meeting at group A: 10 per step, minus the call's first
     ref = oracle_run(w, 3, 4)
     check_amps(ts.get_state(), ref)
     assert np.max(np.abs(ts.expect_all(B.Z) - O.expect_all(ref, N, 2))) <= OBS_TOL
