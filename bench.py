@@ -319,6 +319,31 @@ def run_ours(args):
     ms = float(np.median(region_ms))
     steps_per_s = R.whole_job_steps_per_s(args.steps, world, ms)
 
+    # ---- observable reductions, timed one by one with CUDA events: read-only passes over the state
+    observables = None
+    if args.observables:
+        ts.set_profiling(False)
+        observables = {}
+
+        def timed(name, fn, passes):
+            fn()                                     # warm-up (allocates scratch)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            t = a.elapsed_time(b)
+            observables[name] = {"ms": t, "state_reads": passes, "gbs": passes * 16.0 * dim / (t * 1e-3) / 1e9}
+        ngroups = ts.describe_plan().count("H[") + 1 if "tiled" in ts.describe_plan() else N
+        timed("norm2", ts.norm2, 1)
+        timed("expect_all_z", lambda: ts.expect_all(B.Z), 1)
+        timed("expect_all_x", lambda: ts.expect_all(B.X), ngroups)
+        timed("expect_x_site0", lambda: ts.expect(B.X, 0), 1)
+        timed("correlate_zz", lambda: ts.correlate(B.Z, 0, N - 1), 1)
+        timed("correlate_xx", lambda: ts.correlate(B.X, 0, N - 1), 1)
+        timed("total_sz", ts.total_sz, 1)
+
     # ---- end to end through the C ABI with host buffers: H2D of the state + 1 step + D2H of <S^z_j>
     e2e = None
     if not args.no_e2e:
@@ -403,6 +428,8 @@ def run_ours(args):
            "norm2_after": norm2, "library": B.version(), "kernel_sources_hash": kernel_sources_hash(),
            "gpu_launches": launches, "kernels": kern, "clocks": clocks, "roofline": roofline,
            "cpu_baseline": cpu, "e2e": e2e}
+    if observables is not None:
+        out["observables"] = observables
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -423,6 +450,7 @@ def main():
     ap.add_argument("--config", default="", help="time BASELINE config 1..5 instead of the metric workload")
     ap.add_argument("--repeats", type=int, default=5, help="timed regions of K steps each; the value is their median")
     ap.add_argument("--cpu-full", action="store_true", help="oracle: 3 steps (median) at N = 27 instead of 1")
+    ap.add_argument("--observables", action="store_true", help="also time the observable reductions (row a6)")
     ap.add_argument("--device-state", action="store_true",
                     help="initial state generated on the device (eq. A.1) instead of the seeded host state: for ncu / tuning runs")
     ap.add_argument("--no-e2e", action="store_true")

@@ -161,9 +161,11 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  *                          amplitude), built on first use -- the A/B experiment of DESIGN.md 7.5
  *   TS_OPT_MAX_CTAS        upper bound on the grid of the persistent tile kernels (0, default: one CTA per SM); small values
  *                          make every CTA walk many tiles -- used by the tests to exercise buffer reuse at small N
+ *   TS_OPT_L2_HINTS        1 (default): the L2-blocked launch marks its TMA transfers with L2 eviction priorities (a chunk's
+ *                          intermediate writes "evict last", its final writes and first reads "evict first"); 0: none
  * Errors: TS_ERR_ARG (unknown key, value out of range). */
 enum { TS_OPT_KERNEL = 0, TS_OPT_CHUNK = 1, TS_OPT_CHUNK_MAX_LOG2 = 2, TS_OPT_L2_PROMOTION = 3, TS_OPT_SMALL = 4,
-       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6 };
+       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7 };
 int ts_set_option(ts_ctx* ctx, int key, int value);
 int ts_get_option(ts_ctx* ctx, int key, int* value);
 

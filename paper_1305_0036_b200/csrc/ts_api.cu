@@ -206,6 +206,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->opt_diag_source = 0;
     c->opt_l2_promotion = env_int("TS_L2_PROMOTION", 0);
     c->opt_max_ctas = 0;
+    c->opt_l2_hints = env_int("TS_L2_HINTS", 1);
     c->d_chunk_ctr = nullptr; c->chunk_ctr_cap = 0;
     c->d_energy[0] = c->d_energy[1] = c->d_energy[2] = nullptr;
     c->tmap_psi = nullptr;
@@ -348,11 +349,12 @@ int ts_set_option(ts_ctx* c, int key, int value)
 {
     if (!c) return TS_ERR_ARG;
     switch (key) {
-    case TS_OPT_KERNEL: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_kernel = value; break;
+    case TS_OPT_KERNEL: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_kernel = value; break;
     case TS_OPT_CHUNK: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_chunk = value; break;
     case TS_OPT_CHUNK_MAX_LOG2: if (value < TS_TILE_LOG2 + 1 || value > 26) return TS_ERR_ARG; c->opt_chunk_max_log2 = value; break;
     case TS_OPT_L2_PROMOTION: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_l2_promotion = value; c->tmaps.clear(); break;
     case TS_OPT_MAX_CTAS: if (value < 0) return TS_ERR_ARG; c->opt_max_ctas = value; break;
+    case TS_OPT_L2_HINTS: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_l2_hints = value; break;
     case TS_OPT_DIAG_SOURCE:
         if (value < 0 || value > 1) return TS_ERR_ARG;
         c->opt_diag_source = value;
@@ -382,6 +384,7 @@ int ts_get_option(ts_ctx* c, int key, int* value)
     case TS_OPT_SMALL: *value = c->opt_small; break;
     case TS_OPT_DIAG_SOURCE: *value = c->opt_diag_source; break;
     case TS_OPT_MAX_CTAS: *value = c->opt_max_ctas; break;
+    case TS_OPT_L2_HINTS: *value = c->opt_l2_hints; break;
     default: return TS_ERR_ARG;
     }
     return TS_OK;
@@ -453,7 +456,7 @@ int ts_describe_plan(ts_ctx* c, char* buf, int buflen)
             else snprintf(tmp, sizeof tmp, " H[spins %d..%d, run 2^%d]", t.g0, t.g0 + TS_TILE_LOG2 - t.s - 1, t.s);
             s += tmp;
         }
-        snprintf(tmp, sizeof tmp, "; kernels=%s", c->opt_kernel ? "v2" : "v1");
+        snprintf(tmp, sizeof tmp, "; kernels=%s", c->opt_kernel == 2 ? "v3" : c->opt_kernel ? "v2" : "v1");
         s += tmp;
         if (ts_tile_chunk_supported(c, 1, SW_YDAG, SW_Y)) {
             const TileGroup& t = c->groups[1];

@@ -81,6 +81,7 @@ struct ts_ctx {
     int opt_diag_source;                 // 0: factorised on-the-fly tables, 1: stored 2^N phase vectors, naive plan only
     int opt_l2_promotion;                // tensor-map L2 promotion of the high groups: 0 none, 1 128 B, 2 256 B
     int opt_max_ctas;                    // upper bound on the persistent kernels' grid (0: one CTA per SM)
+    int opt_l2_hints;                    // L2 eviction priorities on the TMA transfers of the L2-blocked launch
     unsigned int* d_chunk_ctr;           // done counters of the triple launch
     size_t chunk_ctr_cap;
     std::vector<TensorMapSlot> tmaps;    // per group, for the bound state pointer tmap_psi

@@ -8,13 +8,15 @@
 
 #include <mutex>
 
-#include "ts_tile_v2.cuh"
+#include "ts_tile_v3.cuh"
 
 namespace {
 
 tile_kernel_t g_tab[5][5];                 // k_tile_pass, run-time butterfly masks
 v2_kernel_t g_v2[3][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits
 v2_chunk_kernel_t g_v2_chunk[2][2];        // [9-bit high group][(Y^dag, Y), (X, X^dag)]
+v2_kernel_t g_v3[3][5][5];                 // the same for the 16-amplitudes-per-thread family (ts_tile_v3.cuh)
+v2_chunk_kernel_t g_v3_chunk[2][2];
 PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
 std::once_flag g_once;
 cudaError_t g_init_status = cudaSuccess;
@@ -24,7 +26,9 @@ cudaError_t g_init_status = cudaSuccess;
 struct PhaseGeom {
     double t;
     int N, nfixed;
-    int rspin[5], tspin[7], xspin[TS_MAX_FIXED];
+    int nr, nt;          // register bits / thread bits at diagonal time (5 + 7, or 4 + 8 for the v3 kernels)
+    int rec;             // entries of a tile-phase record: 32 (nr = 5) or 40 (nr = 4)
+    int rspin[5], tspin[8], xspin[TS_MAX_FIXED];
 };
 
 inline int spin_of_fbit(const TileGroup& g, int f) { return f < g.s ? f : g.g0 + (f - g.s); }
@@ -34,11 +38,15 @@ inline bool v2_geometry_ok(const TileGroup& g) { return g.is_low || (g.s >= 3 &&
 inline int nib(uint32_t pack, int i) { return (int)((pack >> (4 * i)) & 15u); }
 inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : 1); }     // kernel table index
 
-// layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2, H2 or H1).
+// layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2, H2 or H1).  layout 2: v3
+// (ts_tile_v3.cuh: A3, H2 or H1; four register bits, eight thread bits).
 PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
 {
     PhaseGeom q;
     q.t = t; q.N = c->N; q.nfixed = c->N - TS_TILE_LOG2;
+    q.nr = (layout == 2) ? 4 : 5; q.nt = TS_TILE_LOG2 - q.nr; q.rec = (layout == 2) ? TS_V3_REC : 32;
+    for (int b = 0; b < 5; ++b) q.rspin[b] = 0;
+    for (int b = 0; b < 8; ++b) q.tspin[b] = 0;
     const bool two = two_stage(g);
     if (layout == 0) {
         for (int b = 0; b < 5; ++b) q.rspin[b] = spin_of_fbit(g, two ? 2 + b : 7 + b);
@@ -46,11 +54,17 @@ PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
             const int f = two ? (b < 2 ? b : 5 + b) : b;     // layout 2: thread bits 0,1 -> f 0,1; 2..6 -> f 7..11
             q.tspin[b] = spin_of_fbit(g, f);
         }
-    } else {
+    } else if (layout == 1) {
         const uint32_t RP = g.is_low ? TS_V2_A2_R : (two ? TS_V2_H2_R : TS_V2_H1_R);
         const uint32_t TP = g.is_low ? TS_V2_A2_T : (two ? TS_V2_H2_T : TS_V2_H1_T);
         for (int b = 0; b < 5; ++b) q.rspin[b] = spin_of_fbit(g, nib(RP, b));
         for (int b = 0; b < 7; ++b) q.tspin[b] = spin_of_fbit(g, nib(TP, b));
+    } else {
+        const bool two3 = !g.is_low && n_bfly(g) > 4;
+        const uint32_t RP = g.is_low ? TS_V3_A3_R : (two3 ? TS_V3_H2_R : TS_V3_H1_R);
+        const uint32_t TP = g.is_low ? TS_V3_A3_T : (two3 ? TS_V3_H2_T : TS_V3_H1_T);
+        for (int b = 0; b < 4; ++b) q.rspin[b] = spin_of_fbit(g, nib(RP, b));
+        for (int b = 0; b < 8; ++b) q.tspin[b] = spin_of_fbit(g, nib(TP, b));
     }
     bool in_tile[TS_MAX_N] = {false};
     for (int f = 0; f < TS_TILE_LOG2; ++f) in_tile[spin_of_fbit(g, f)] = true;
@@ -60,35 +74,38 @@ PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
     return q;
 }
 
-// TT[v], WT[0..4][v] for thread index v (one block of 128 threads).
-__global__ void __launch_bounds__(128) k_build_thread_tables(double2* __restrict__ out, const PhaseGeom q,
+// TT[v], WT[0..nr-1][v] for thread index v (one block of 2^nt threads); out = TT[2^nt] followed by WT[nr][2^nt].
+__global__ void __launch_bounds__(256) k_build_thread_tables(double2* __restrict__ out, const PhaseGeom q,
                                                              const double* __restrict__ h,
                                                              const double* __restrict__ Jeff)
 {
     const int v = threadIdx.x;
-    double sg[7];
-    for (int b = 0; b < 7; ++b) sg[b] = (double)((v >> b) & 1) - 0.5;
+    const int GT = 1 << q.nt;
+    double sg[8];
+    for (int b = 0; b < q.nt; ++b) sg[b] = (double)((v >> b) & 1) - 0.5;
     double ET = 0.0;                              // fields and couplings among the thread spins
-    for (int b = 0; b < 7; ++b) {
+    for (int b = 0; b < q.nt; ++b) {
         double f = h[q.tspin[b]];
         for (int c = 0; c < b; ++c) f += Jeff[q.tspin[b] * TS_MAX_N + q.tspin[c]] * sg[c];
         ET += sg[b] * f;
     }
     double bsum = 0.0;
-    for (int i = 0; i < 5; ++i) {
+    for (int i = 0; i < q.nr; ++i) {
         double bi = 0.0;
-        for (int b = 0; b < 7; ++b) bi += Jeff[q.rspin[i] * TS_MAX_N + q.tspin[b]] * sg[b];
+        for (int b = 0; b < q.nt; ++b) bi += Jeff[q.rspin[i] * TS_MAX_N + q.tspin[b]] * sg[b];
         bsum += bi;
         double sn, cs;
         sincos(-q.t * bi, &sn, &cs);
-        out[128 + i * 128 + v] = make_double2(cs, sn);
+        out[GT + i * GT + v] = make_double2(cs, sn);
     }
     double sn, cs;
     sincos(-q.t * (ET - 0.5 * bsum), &sn, &cs);
     out[v] = make_double2(cs, sn);
 }
 
-// Tile-phase table: 32 entries per tile (layout in ts_tile_kernel.cuh); one thread per entry.
+// Tile-phase table: q.rec entries per tile, one thread per entry:
+//   [0] tp0;  [1..16] the four low thread bits;  [17 .. 16 + 2^(nt-4)] the remaining thread bits;  then nr entries tpW;
+//   the rest is padding (1).  (Layout and meaning in ts_tile_kernel.cuh.)
 __global__ void __launch_bounds__(256) k_build_tile_phase(double2* __restrict__ out, uint64_t ntiles,
                                                           const PhaseGeom q, const double* __restrict__ h,
                                                           const double* __restrict__ Jeff)
@@ -99,10 +116,11 @@ __global__ void __launch_bounds__(256) k_build_tile_phase(double2* __restrict__ 
     for (int i = threadIdx.x; i < TS_MAX_N; i += blockDim.x) sh[i] = h[i];
     __syncthreads();
     const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t tau = gid >> 5;
-    const int e = (int)(gid & 31);
+    const uint64_t tau = gid / (uint64_t)q.rec;
+    const int e = (int)(gid % (uint64_t)q.rec);
     if (tau >= ntiles) return;
     const int nf = q.nfixed;
+    const int nhi = q.nt - 4, wofs = 17 + (1 << nhi);
     auto a_of = [&](int j) {                      // a_j(tau) = sum_x Jeff_jx sigma_x(tau)
         double a = 0.0;
         for (int x = 0; x < nf; ++x) a = fma(sJ[j * TS_MAX_N + q.xspin[x]], (double)((tau >> x) & 1) - 0.5, a);
@@ -115,16 +133,16 @@ __global__ void __launch_bounds__(256) k_build_tile_phase(double2* __restrict__ 
             E = fma((double)((tau >> x) & 1) - 0.5, sh[sp] + 0.5 * a_of(sp), E);
         }
         double ar = 0.0;
-        for (int i = 0; i < 5; ++i) ar += a_of(q.rspin[i]);
+        for (int i = 0; i < q.nr; ++i) ar += a_of(q.rspin[i]);
         E -= 0.5 * ar;
     } else if (e < 17) {
         const int v = e - 1;
         for (int b = 0; b < 4; ++b) E = fma((double)((v >> b) & 1) - 0.5, a_of(q.tspin[b]), E);
-    } else if (e < 25) {
+    } else if (e < wofs) {
         const int v = e - 17;
-        for (int b = 0; b < 3; ++b) E = fma((double)((v >> b) & 1) - 0.5, a_of(q.tspin[4 + b]), E);
-    } else if (e < 30) {
-        E = a_of(q.rspin[e - 25]);
+        for (int b = 0; b < nhi; ++b) E = fma((double)((v >> b) & 1) - 0.5, a_of(q.tspin[4 + b]), E);
+    } else if (e < wofs + q.nr) {
+        E = a_of(q.rspin[e - wofs]);
     }
     double sn, cs;
     sincos(-q.t * E, &sn, &cs);
@@ -136,9 +154,11 @@ __global__ void __launch_bounds__(256) k_build_tile_phase(double2* __restrict__ 
 // later re-normalisation, so a common modulus bias of ~1e-17 would add up linearly in the norm.
 void build_RR(const ts_ctx* c, const PhaseGeom& q, int alpha, double2* RR)
 {
-    for (int r = 0; r < 32; ++r) {
+    const int nrr = 1 << q.nr;
+    for (int r = nrr; r < 32; ++r) RR[r] = make_double2(1.0, 0.0);
+    for (int r = 0; r < nrr; ++r) {
         double ER = 0.0;
-        for (int i = 0; i < 5; ++i) {
+        for (int i = 0; i < q.nr; ++i) {
             const double si = (double)((r >> i) & 1) - 0.5;
             double f = c->h[alpha][q.rspin[i]];
             for (int k = 0; k < i; ++k) f += c->Jeff[alpha][q.rspin[i]][q.rspin[k]] * ((double)((r >> k) & 1) - 0.5);
@@ -147,7 +167,7 @@ void build_RR(const ts_ctx* c, const PhaseGeom& q, int alpha, double2* RR)
         RR[r] = make_double2(cos(-q.t * ER), sin(-q.t * ER));
     }
     double S = 0.0;
-    for (int r = 0; r < 32; ++r) {
+    for (int r = 0; r < nrr; ++r) {
         const double2 z = RR[r];
         double best = 0.0; double2 zb = z; bool have = false;
         for (int cand = 0; cand < 3; ++cand) {
@@ -182,6 +202,16 @@ void init_once()
     ts_v2_register_chunk1(g_v2_chunk);
     ts_v2_register_chunk0_h9(g_v2_chunk);
     ts_v2_register_chunk1_h9(g_v2_chunk);
+    memset(g_v3, 0, sizeof(g_v3));
+    ts_v3_register_A(&g_v3[0]);
+    ts_v3_register_Hf(&g_v3[1]);
+    ts_v3_register_Hs(&g_v3[1]);
+    ts_v3_register_H9(&g_v3[2]);
+    memset(g_v3_chunk, 0, sizeof(g_v3_chunk));
+    ts_v3_register_chunk0(g_v3_chunk);
+    ts_v3_register_chunk1(g_v3_chunk);
+    ts_v3_register_chunk0_h9(g_v3_chunk);
+    ts_v3_register_chunk1_h9(g_v3_chunk);
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
@@ -197,6 +227,15 @@ void init_once()
         for (int v = 0; v < 2 && e == cudaSuccess; ++v)
             if (g_v2_chunk[hm][v])
                 e = cudaFuncSetAttribute((const void*)g_v2_chunk[hm][v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
+    for (int ty = 0; ty < 3 && e == cudaSuccess; ++ty)
+        for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
+            for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
+                if (g_v3[ty][k1][k2])
+                    e = cudaFuncSetAttribute((const void*)g_v3[ty][k1][k2], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V3_SMEM);
+    for (int hm = 0; hm < 2 && e == cudaSuccess; ++hm)
+        for (int v = 0; v < 2 && e == cudaSuccess; ++v)
+            if (g_v3_chunk[hm][v])
+                e = cudaFuncSetAttribute((const void*)g_v3_chunk[hm][v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V3_SMEM);
     for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
         for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
             if (g_tab[k1][k2])
@@ -228,17 +267,18 @@ void fill_v1_params(const ts_ctx* c, const TileGroup& g, const DiagTables* tb, T
     else { p->bf1 = 31u; p->bf2 = (31u << (10 - nb)) & 31u; }                       // top nb-5 bits of f 2..6
 }
 
-void fill_v2_geom(const TileGroup& g, V2Geom* q)
+// family: 1 = v2 (32 amplitudes per thread), 2 = v3 (16)
+void fill_v2_geom(const TileGroup& g, int family, V2Geom* q)
 {
     q->type = g.is_low ? 0 : 1;
     q->s = g.s; q->g0 = g.g0;
     q->m = g.is_low ? 0 : TS_TILE_LOG2 - g.s;
     q->nmid = g.g0 - g.s;
-    q->two_stage = (!g.is_low && q->m > 5) ? 1 : 0;
+    q->two_stage = (!g.is_low && q->m > (family == 2 ? 4 : 5)) ? 1 : 0;
     q->mask1 = 0u; q->mask2 = 0u;
     if (!g.is_low) {
-        q->mask1 = tsk::v2_h_mask1(q->m);
-        q->mask2 = tsk::v2_h_mask2(q->m);     // H2 register bit 4 (f 7) is a filler: f 7 was butterflied in H1
+        q->mask1 = family == 2 ? v3_h_mask1(q->m) : tsk::v2_h_mask1(q->m);
+        q->mask2 = family == 2 ? v3_h_mask2(q->m) : tsk::v2_h_mask2(q->m);   // (v2: H2 register bit 4 = f 7 is a filler)
     }
 }
 
@@ -328,24 +368,26 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, int layout
     const TileGroup& g = c->groups[group];
     const PhaseGeom q = make_geom(c, g, d.t, layout);
     const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
+    const int GT = 1 << q.nt, nrr = 1 << q.nr;
+    const size_t n_thread_tab = (size_t)(1 + q.nr) * GT;          // TT, WT[nr]; RR[2^nr] follows
     DiagTables* tb = new DiagTables();
     tb->alpha = d.alpha; tb->scale_pow = d.scale_pow; tb->group = group; tb->layout = layout; tb->t = d.t;
     tb->d_thread = nullptr; tb->d_tile_phase = nullptr;
-    cudaError_t e = cudaMalloc(&tb->d_thread, sizeof(double2) * (6 * 128 + 32));     // TT, WT[5], RR
-    if (e == cudaSuccess) e = cudaMalloc(&tb->d_tile_phase, sizeof(double2) * 32 * ntiles);
+    cudaError_t e = cudaMalloc(&tb->d_thread, sizeof(double2) * (n_thread_tab + nrr));
+    if (e == cudaSuccess) e = cudaMalloc(&tb->d_tile_phase, sizeof(double2) * (size_t)q.rec * ntiles);
     if (e != cudaSuccess) {
         if (tb->d_thread) cudaFree(tb->d_thread);
         delete tb;
         return e;
     }
     build_RR(c, q, d.alpha, tb->RR);
-    e = cudaMemcpyAsync(tb->d_thread + 6 * 128, tb->RR, sizeof(tb->RR), cudaMemcpyHostToDevice, c->stream);   // (tb is heap-allocated and lives as long as the cache entry)
+    e = cudaMemcpyAsync(tb->d_thread + n_thread_tab, tb->RR, sizeof(double2) * nrr, cudaMemcpyHostToDevice, c->stream);   // (tb is heap-allocated and lives as long as the cache entry)
     if (e != cudaSuccess) { cudaFree(tb->d_thread); cudaFree(tb->d_tile_phase); delete tb; return e; }
     const double* dh = c->d_h + d.alpha * TS_MAX_N;
     const double* dJ = c->d_Jeff + (size_t)d.alpha * TS_MAX_N * TS_MAX_N;
     ts_prof_begin(c, TS_KC_SETUP);
-    k_build_thread_tables<<<1, 128, 0, c->stream>>>(tb->d_thread, q, dh, dJ);
-    const uint64_t nthreads = ntiles * 32;
+    k_build_thread_tables<<<1, GT, 0, c->stream>>>(tb->d_thread, q, dh, dJ);
+    const uint64_t nthreads = ntiles * (uint64_t)q.rec;
     k_build_tile_phase<<<(unsigned)((nthreads + 255) / 256), 256, 0, c->stream>>>(tb->d_tile_phase, ntiles, q, dh, dJ);
     ts_prof_end(c);
     c->launches[TS_KC_SETUP]++;
@@ -359,6 +401,7 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
 {
     const TileGroup& g = c->groups[group];
     if (c->opt_kernel == 0 || !v2_geometry_ok(g)) return 0;
+    if (c->opt_kernel == 2) return g_v3[v2_type(g)][kind1][kind2] ? 2 : 0;
     return g_v2[v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
@@ -373,9 +416,9 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
     }
     const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
     const bool fused = (kind1 != SW_NONE && kind2 != SW_NONE);
-    if (layout == 1) {
+    if (layout >= 1) {
         V2Pass p;
-        fill_v2_geom(g, &p.g);
+        fill_v2_geom(g, layout, &p.g);
         fill_v2_diag(tb, &p.d);
         p.ntiles = ntiles;
         CUtensorMap tm;
@@ -384,7 +427,8 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
         const uint64_t cap = (c->opt_max_ctas > 0 && c->opt_max_ctas < c->num_sms) ? (uint64_t)c->opt_max_ctas : (uint64_t)c->num_sms;
         const uint64_t grid = ntiles < cap ? ntiles : cap;
         ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
-        g_v2[v2_type(g)][kind1][kind2]<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
+        if (layout == 2) g_v3[v2_type(g)][kind1][kind2]<<<(unsigned)grid, TS_V3_THREADS, TS_V3_SMEM, c->stream>>>(p, tm);
+        else g_v2[v2_type(g)][kind1][kind2]<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
         ts_prof_end(c);
         return cudaGetLastError();
     }
@@ -408,7 +452,7 @@ bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
     if (C >= c->N || C > c->opt_chunk_max_log2) return false;          // at least two chunks, each small enough for L2
     const int v = (ka == SW_YDAG && kb == SW_Y) ? 0 : (ka == SW_X && kb == SW_XDAG) ? 1 : -1;
-    return v >= 0 && g_v2_chunk[g.s == 3 ? 1 : 0][v] != nullptr;
+    return v >= 0 && (c->opt_kernel == 2 ? g_v3_chunk : g_v2_chunk)[g.s == 3 ? 1 : 0][v] != nullptr;
 }
 
 cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int kb)
@@ -418,8 +462,9 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
     const uint32_t nchunks = 1u << (c->N - C);
     const DiagTables* tb = nullptr;
     cudaError_t e = cudaSuccess;
+    const int family = (c->opt_kernel == 2) ? 2 : 1;
     if (d.present) {
-        e = ts_tile_get_tables(c, d, 0, 1, &tb);
+        e = ts_tile_get_tables(c, d, 0, family, &tb);
         if (e != cudaSuccess) return e;
     }
     const size_t nctr = 2 * (size_t)nchunks;
@@ -433,11 +478,12 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
         c->chunk_ctr_cap = nctr;
     }
     V2Chunk q;
-    fill_v2_geom(g, &q.gh);
-    fill_v2_geom(c->groups[0], &q.ga);
+    fill_v2_geom(g, family, &q.gh);
+    fill_v2_geom(c->groups[0], family, &q.ga);
     fill_v2_diag(tb, &q.d);
     q.done = c->d_chunk_ctr;
     q.nchunks = nchunks; q.tiles_log2 = (uint32_t)(C - TS_TILE_LOG2);
+    q.l2_hints = c->opt_l2_hints;
     e = cudaMemsetAsync(c->d_chunk_ctr, 0, sizeof(unsigned int) * nctr, c->stream);
     if (e != cudaSuccess) return e;
     CUtensorMap tmA, tmH;
@@ -451,7 +497,12 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
     ts_prof_begin(c, TS_KC_TILE_CHUNK, 3.0);
     // cooperative launch: the loaders wait on other CTAs' progress, so all CTAs must be resident (else: error, not a hang)
     void* args[3] = {(void*)&q, (void*)&tmA, (void*)&tmH};
-    e = cudaLaunchCooperativeKernel((const void*)g_v2_chunk[g.s == 3 ? 1 : 0][v], dim3((unsigned)grid), dim3(TS_V2_THREADS), args, TS_V2_SMEM, c->stream);
+    if (family == 2)
+        e = cudaLaunchCooperativeKernel((const void*)g_v3_chunk[g.s == 3 ? 1 : 0][v], dim3((unsigned)grid), dim3(TS_V3_THREADS), args,
+                                        TS_V3_SMEM, c->stream);
+    else
+        e = cudaLaunchCooperativeKernel((const void*)g_v2_chunk[g.s == 3 ? 1 : 0][v], dim3((unsigned)grid), dim3(TS_V2_THREADS), args,
+                                        TS_V2_SMEM, c->stream);
     ts_prof_end(c);
     return e;
 }

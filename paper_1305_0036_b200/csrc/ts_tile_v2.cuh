@@ -78,6 +78,7 @@ struct V2Chunk {
     V2Diag d;
     unsigned int* done;          // [2][nchunks] tiles finished (and globally visible) of phase 1 / phase 2 of a chunk
     uint32_t nchunks, tiles_log2;
+    int l2_hints;                // 1: eviction priorities on the TMA transfers (keep a chunk in L2 until its third phase wrote it)
 };
 
 typedef void (*v2_kernel_t)(const V2Pass, const CUtensorMap);
@@ -156,6 +157,42 @@ __device__ __forceinline__ void v2_tma_store_4d(const CUtensorMap* tm, uint32_t 
 {
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(tm), "r"(src),
                  "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+                 : "memory");
+}
+// L2 eviction-priority policies for the L2-blocked launch (createpolicy; 0: evict_normal, 1: evict_first, 2: evict_last)
+__device__ __forceinline__ uint64_t v2_policy(int kind)
+{
+    uint64_t pol;
+    if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void v2_tma_load_2d_h(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(dst),
+        "l"(tm), "r"(bar), "r"(c0), "r"(c1), "l"(pol)
+        : "memory");
+}
+__device__ __forceinline__ void v2_tma_load_4d_h(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2, int c3,
+                                                 uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], [%2], %7;" ::"r"(dst),
+        "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol)
+        : "memory");
+}
+__device__ __forceinline__ void v2_tma_store_2d_h(const CUtensorMap* tm, uint32_t src, int c0, int c1, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;" ::"l"(tm),
+                 "r"(src), "r"(c0), "r"(c1), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void v2_tma_store_4d_h(const CUtensorMap* tm, uint32_t src, int c0, int c1, int c2, int c3, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%2, %3, %4, %5}], [%1], %6;" ::"l"(tm),
+                 "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol)
                  : "memory");
 }
 __device__ __forceinline__ void v2_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
@@ -375,6 +412,32 @@ __device__ __forceinline__ void v2_issue_load(const V2Geom& g, const CUtensorMap
         v2_tma_load_4d(dst + 32768u, tm, bar, 0, c1, c2hi, c3);
     }
 }
+__device__ __forceinline__ void v2_issue_load_h(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t dst,
+                                                const uint32_t bar, const uint64_t pol)
+{
+    int c1, c2lo, c2hi, c3;
+    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
+    if (g.type == 0) {
+        v2_tma_load_2d_h(dst, tm, bar, 0, c1 + c2lo, pol);
+        v2_tma_load_2d_h(dst + 32768u, tm, bar, 0, c1 + c2hi, pol);
+    } else {
+        v2_tma_load_4d_h(dst, tm, bar, 0, c1, c2lo, c3, pol);
+        v2_tma_load_4d_h(dst + 32768u, tm, bar, 0, c1, c2hi, c3, pol);
+    }
+}
+__device__ __forceinline__ void v2_issue_store_h(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src,
+                                                 const uint64_t pol)
+{
+    int c1, c2lo, c2hi, c3;
+    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
+    if (g.type == 0) {
+        v2_tma_store_2d_h(tm, src, 0, c1 + c2lo, pol);
+        v2_tma_store_2d_h(tm, src + 32768u, 0, c1 + c2hi, pol);
+    } else {
+        v2_tma_store_4d_h(tm, src, 0, c1, c2lo, c3, pol);
+        v2_tma_store_4d_h(tm, src + 32768u, 0, c1, c2hi, c3, pol);
+    }
+}
 __device__ __forceinline__ void v2_issue_store(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src)
 {
     int c1, c2lo, c2hi, c3;
@@ -533,6 +596,9 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
                 v2_mbar_expect_tx(sBar + 8 * 3 * TS_V2_NBUF, TS_V2_TAB_BYTES);
                 v2_bulk_load(sBase + TS_V2_OFF_TAB, q.d.tables, TS_V2_TAB_BYTES, sBar + 8 * 3 * TS_V2_NBUF);
             }
+            // L2 priorities: what phase 1 reads from HBM is about to be overwritten (evict first); what phases 1 and 2
+            // write is read again from L2 (evict last); the third phase's reads are the last use of a line.
+            const uint64_t pol_ld[3] = {v2_policy(q.l2_hints ? 1 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
             uint32_t ok_key = 0xffffffffu;             // (phase, chunk) whose dependency was last seen satisfied
             for (uint64_t j = 0; j < n_cta; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
@@ -552,27 +618,28 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
                 const bool tpl = has_diag && phase == 1;
                 v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (tpl ? 512u : 0u));
                 if (tpl) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, q.d.tile_phase + (tile << 5), 512u, bar);
-                if (phase == 1) v2_issue_load(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, bar);
-                else v2_issue_load(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+                if (phase == 1) v2_issue_load_h(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[1]);
+                else v2_issue_load_h(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[phase]);
             }
         } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
+            const uint64_t pol_st[3] = {v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
             for (uint64_t j = 0; j < n_cta; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
                 uint32_t phase, c; uint64_t tile;
                 job_of(j, phase, c, tile);
                 v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
-                if (phase == 1) v2_issue_store(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES);
-                else v2_issue_store(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES);
+                if (phase == 1) v2_issue_store_h(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[1]);
+                else v2_issue_store_h(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[phase]);
                 v2_store_commit();
+                v2_store_wait_read();                  // the buffer can be refilled as soon as the store has read it
+                v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
                 if (phase != 2) {
-                    v2_store_wait_all();               // the tile is in global memory (L2) ...
-                    v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
+                    // Publish only once the tile IS in global memory (L2).  (Not deferred to the next job: a publish
+                    // that waited for this CTA's next job could wait for a job that depends on it.)
+                    v2_store_wait_all();
                     v2_fence_async_all();
-                    __threadfence();                   // ... before it is published to the other CTAs' loaders
+                    __threadfence();
                     atomicAdd(q.done + (size_t)phase * q.nchunks + c, 1u);
-                } else {
-                    v2_store_wait_read();
-                    v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
                 }
             }
             v2_store_wait_all();

@@ -158,12 +158,17 @@ def test_config2_ring16_trace(B):
         ref.append(O.expect(psi, w.N, 2, 0))
     assert np.max(np.abs(np.array(got) - np.array(ref))) <= OBS_TOL
     check_amps(ts.get_state(), psi)
-    assert abs(ts.norm2() - 1.0) <= 1e-13
+    # 200 separate steps = 8 000 diagonals; each multiplies an amplitude by a table product whose modulus is 1 up to a few
+    # ulp that are FIXED per (tile, thread, register): starting from a basis state nothing averages them out at first.
+    # Bound: 8 000 x 2 x 3e-17 = 5e-13; the oracle's own norm is held to 1e-13 by tests/test_oracle_pins.py.
+    assert abs(ts.norm2() - 1.0) <= 5e-13
 
 
-def test_config3_dipolar22(B):
+def test_config3_dipolar22_all_100_steps(B):
+    """BASELINE config 3 at its configured 100 steps (the oracle needs ~1 s per step at N = 22 on the box's 16 cores)."""
     w = W.config(3)
-    n = w.n_steps if FULL else 8
+    n = w.n_steps
+    assert n == 100
     ts = run_gpu(B, w, n_steps=n)
     ref = run_oracle(w, n_steps=n)
     check_amps(ts.get_state(), ref)

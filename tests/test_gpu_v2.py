@@ -63,12 +63,17 @@ TRIPLE_CASES = [
 ]
 
 
+FAMILIES = [1, 2]      # TS_OPT_KERNEL: 32 amplitudes per thread (ts_tile_v2.cuh), 16 (ts_tile_v3.cuh)
+
+
 @pytest.mark.parametrize("N,groups", TRIPLE_CASES)
 @pytest.mark.parametrize("order", [4, 2])
-def test_triple_launch_generic_J_full_oracle(B, N, groups, order):
+@pytest.mark.parametrize("family", FAMILIES)
+def test_triple_launch_generic_J_full_oracle(B, N, groups, order, family):
     steps = 3 if N <= 22 else 2
     w = W.generic(N, seed=500 + 7 * N + len(groups) + order, tau=0.02, n_steps=steps, order=order, symmetric_fill=(N % 3 == 0))
     ts = B.TrotterSuzuki(N, w.h, w.J)
+    ts.set_option(B.OPT_KERNEL, family)
     ts.set_plan_groups(groups)
     ts.set_state(w.state())
     ts.reset_profile()
@@ -81,11 +86,13 @@ def test_triple_launch_generic_J_full_oracle(B, N, groups, order):
     ts.close()
 
 
-def test_default_plan_N24_triple_launch_three_steps(B):
+@pytest.mark.parametrize("family", FAMILIES)
+def test_default_plan_N24_triple_launch_three_steps(B, family):
     """The default plan (A + 9 + rest) at N = 24 against the full oracle: the bench plan's geometry with 8 chunks."""
     N = 24
     w = W.generic(N, seed=2424, tau=0.02, n_steps=3)
     ts = B.TrotterSuzuki(N, w.h, w.J)
+    ts.set_option(B.OPT_KERNEL, family)
     ts.set_state(w.state())
     ts.reset_profile()
     ts.evolve(w.tau, 3, 4)
@@ -104,7 +111,7 @@ def test_kernel_families_agree_and_match_oracle(B, N, groups):
     kernels: each against the oracle."""
     w = W.generic(N, seed=900 + N, tau=0.02, n_steps=2)
     ref = oracle_run(w, 2, 4)
-    for kernel, chunk in ((1, 1), (1, 0), (0, 0)):
+    for kernel, chunk in ((1, 1), (1, 0), (2, 1), (2, 0), (0, 0)):
         ts = B.TrotterSuzuki(N, w.h, w.J)
         ts.set_plan_groups(groups)
         ts.set_option(B.OPT_KERNEL, kernel)
@@ -122,13 +129,15 @@ def test_kernel_families_agree_and_match_oracle(B, N, groups):
 
 @pytest.mark.parametrize("max_ctas", [1, 2, 3, 5, 148])
 @pytest.mark.parametrize("N,groups", [(16, [4]), (17, [2, 3]), (19, [7]), (18, [3, 3])])
-def test_few_ctas_walk_many_tiles(B, N, groups, max_ctas):
+@pytest.mark.parametrize("family", FAMILIES)
+def test_few_ctas_walk_many_tiles(B, N, groups, max_ctas, family):
     """Persistent kernels with 1..5 CTAs: every CTA runs tens of jobs through its three tile buffers (buffer reuse, the
     loader / storer / compute hand-over at every phase parity, ragged job counts per CTA), with and without the triple
     launch.  Full oracle."""
     w = W.generic(N, seed=800 + N + max_ctas, tau=0.02, n_steps=2)
     ts = B.TrotterSuzuki(N, w.h, w.J)
     ts.set_plan_groups(groups)
+    ts.set_option(B.OPT_KERNEL, family)
     ts.set_option(B.OPT_MAX_CTAS, max_ctas)
     ts.set_state(w.state())
     ts.evolve(w.tau, 2, 4)
@@ -142,6 +151,7 @@ def test_triple_launch_repeated_in_one_process(B):
     for rep in range(30):
         w = W.generic(N, seed=7000 + rep, tau=0.02, n_steps=4)
         ts = B.TrotterSuzuki(N, w.h, w.J)
+        ts.set_option(B.OPT_KERNEL, 1 + (rep // 2) % 2)
         ts.set_plan_groups([2, 4] if rep % 2 else [3, 3])
         ts.set_state(w.state())
         ts.reset_profile()
