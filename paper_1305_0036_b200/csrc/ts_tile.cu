@@ -38,7 +38,7 @@ inline bool v2_geometry_ok(const TileGroup& g) { return g.is_low || (g.s >= 3 &&
 inline int nib(uint32_t pack, int i) { return (int)((pack >> (4 * i)) & 15u); }
 inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : 1); }     // kernel table index
 
-// layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2, H2 or H1).  layout 2: v3
+// layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2', H2 or H1).  layout 2: v3
 // (ts_tile_v3.cuh: A3, H2 or H1; four register bits, eight thread bits).
 PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
 {
@@ -55,8 +55,8 @@ PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
             q.tspin[b] = spin_of_fbit(g, f);
         }
     } else if (layout == 1) {
-        const uint32_t RP = g.is_low ? TS_V2_A2_R : (two ? TS_V2_H2_R : TS_V2_H1_R);
-        const uint32_t TP = g.is_low ? TS_V2_A2_T : (two ? TS_V2_H2_T : TS_V2_H1_T);
+        const uint32_t RP = g.is_low ? TS_V2_A2S_R : (two ? TS_V2_H2_R : TS_V2_H1_R);
+        const uint32_t TP = g.is_low ? TS_V2_A2S_T : (two ? TS_V2_H2_T : TS_V2_H1_T);
         for (int b = 0; b < 5; ++b) q.rspin[b] = spin_of_fbit(g, nib(RP, b));
         for (int b = 0; b < 7; ++b) q.tspin[b] = spin_of_fbit(g, nib(TP, b));
     } else {

@@ -23,8 +23,9 @@
 // register / thread bit):
 //   A1: regs {3,4,5,10,11}  threads {0,1,2,8,9,6,7}        A2: regs {0,1,2,8,9}  threads {3,4,5,6,7,10,11}
 //   H1: regs {7,8,9,10,11}  threads {0,1,2,3,4,5,6}        H2: regs {3,4,5,6,7}  threads {0,1,2,8,9,10,11}
-// Group A butterflies all 12 bits: 5 in A1, 5 in A2 and f6, f7 (lane bits 3, 4 of A2) by warp shuffles; the diagonal is
-// applied in A2.  A high group butterflies f >= s: f7..11 in H1 and f_s..6 in H2 (m > 5 only; diagonal in H2, else H1).
+// Group A butterflies all 12 bits without warp shuffles: K1 on 5 bits in A1, 5 in A2, then A2 -> A2' (regs {0,1,2,6,7}:
+// lane bits 3, 4 swapped with register bits 3, 4 -- an exchange INSIDE each warp's quarter of the buffer, __syncwarp only)
+// and f6, f7 there; the diagonal in A2'; K2 on all five register bits of A2', the five of A1, and f8, f9 in A1'.  A high group butterflies f >= s: f7..11 in H1 and f_s..6 in H2 (m > 5 only; diagonal in H2, else H1).
 #pragma once
 #include <cuda.h>
 
@@ -45,6 +46,12 @@
 #define TS_V2_A1_T 0x7698210u
 #define TS_V2_A2_R 0x98210u
 #define TS_V2_A2_T 0xBA76543u
+// A2' / A1': A2 / A1 with lane bits 3, 4 and register bits 3, 4 swapped (an intra-warp exchange through the warp's own
+// quarter of the tile buffer: no block barrier).  They put f6, f7 (resp. f8, f9) on register bits.
+#define TS_V2_A2S_R 0x76210u
+#define TS_V2_A2S_T 0xBA98543u
+#define TS_V2_A1S_R 0x98543u
+#define TS_V2_A1S_T 0x76BA210u
 #define TS_V2_H1_R 0xBA987u
 #define TS_V2_H1_T 0x6543210u
 #define TS_V2_H2_R 0x76543u
@@ -304,37 +311,40 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, c
 {
     using L1 = V2Layout<TS_V2_A1_R, TS_V2_A1_T>;
     using L2 = V2Layout<TS_V2_A2_R, TS_V2_A2_T>;
-    const int lane = t & 31;
-    const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t);
+    using L1S = V2Layout<TS_V2_A1S_R, TS_V2_A1S_T>;
+    using L2S = V2Layout<TS_V2_A2S_R, TS_V2_A2S_T>;
+    const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t), o1s = L1S::thread_off(t), o2s = L2S::thread_off(t);
     double re[32], im[32];
     if (K1 != SW_NONE) {
         L1::load(buf, o1, re, im);
         bfly_regs<K1, 31>(re, im, 0u);                 // f 3,4,5,10,11
         L1::store(buf, o1, re, im);
         v2_group_sync(grp);
-    }
-    L2::load(buf, o2, re, im);
-    if (K1 != SW_NONE) {
+        L2::load(buf, o2, re, im);
         bfly_regs<K1, 31>(re, im, 0u);                 // f 0,1,2,8,9
-        bfly_lane<K1>(re, im, 3, lane);                // f 6
-        bfly_lane<K1>(re, im, 4, lane);                // f 7
+        L2::store(buf, o2, re, im);                    // A2 -> A2': lanes <-> registers inside the warp's own quarter
+        __syncwarp();
     }
+    L2S::load(buf, o2s, re, im);
+    bfly_regs<K1, 24>(re, im, 0u);                     // f 6,7
     if (diag) {
         double2 base, w[5];
         v2_thread_phase(scale, tp, tab, t, base, w);
         v2_apply_diag(tab + 768, base, w, re, im);
     }
     if (K2 != SW_NONE) {
-        bfly_lane<K2>(re, im, 4, lane);
-        bfly_lane<K2>(re, im, 3, lane);
-        bfly_regs<K2, 31>(re, im, 0u);
-        L2::store(buf, o2, re, im);
+        bfly_regs<K2, 31>(re, im, 0u);                 // f 0,1,2,6,7
+        L2S::store(buf, o2s, re, im);
         v2_group_sync(grp);
         L1::load(buf, o1, re, im);
-        bfly_regs<K2, 31>(re, im, 0u);
-        L1::store(buf, o1, re, im);
+        bfly_regs<K2, 31>(re, im, 0u);                 // f 3,4,5,10,11
+        L1::store(buf, o1, re, im);                    // A1 -> A1'
+        __syncwarp();
+        L1S::load(buf, o1s, re, im);
+        bfly_regs<K2, 24>(re, im, 0u);                 // f 8,9
+        L1S::store(buf, o1s, re, im);
     } else {
-        L2::store(buf, o2, re, im);
+        L2S::store(buf, o2s, re, im);
     }
 }
 
