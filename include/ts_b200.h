@@ -163,9 +163,16 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  *                          make every CTA walk many tiles -- used by the tests to exercise buffer reuse at small N
  *   TS_OPT_L2_HINTS        1 (default): the L2-blocked launch marks its TMA transfers with L2 eviction priorities (a chunk's
  *                          intermediate writes "evict last", its final writes and first reads "evict first"); 0: none
+ *   TS_OPT_PAIR            1 (default): a scheduling ticket of a high-group pass is a pair of adjacent tiles (their 128-byte
+ *                          rows are the halves of 256-byte segments: DRAM page locality); 0: single tiles
+ *   TS_OPT_PROBE           0 (default); 1: MEASUREMENT ONLY -- the tile kernels move every tile through their pipeline (TMA
+ *                          in, TMA out) but skip the arithmetic, so the state is left unchanged by ts_evolve: the copy
+ *                          ceiling of each pass's access pattern (bench.py --opt probe=1); 2 / 3: the fused
+ *                          passes and the (Y^dag, Y) triple launch of the N = 30 plan run with only their arithmetic / only
+ *                          their shared-memory layout exchanges (wrong results by construction; time attribution only)
  * Errors: TS_ERR_ARG (unknown key, value out of range). */
 enum { TS_OPT_KERNEL = 0, TS_OPT_CHUNK = 1, TS_OPT_CHUNK_MAX_LOG2 = 2, TS_OPT_L2_PROMOTION = 3, TS_OPT_SMALL = 4,
-       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7 };
+       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7, TS_OPT_PAIR = 8, TS_OPT_PROBE = 9 };
 int ts_set_option(ts_ctx* ctx, int key, int value);
 int ts_get_option(ts_ctx* ctx, int key, int* value);
 

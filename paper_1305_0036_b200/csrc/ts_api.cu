@@ -171,7 +171,7 @@ const char* ts_strerror(int s)
     }
 }
 
-const char* ts_version(void) { return "ts_b200 0.2 sm_100a tile=2^12 regs=32amp/thread kernels=v2(tma-in/out,warp-specialised)+v1"; }
+const char* ts_version(void) { return "ts_b200 0.3 sm_100a tile=2^12 regs=32amp/thread kernels=v2(tma-in/out,warp-specialised,ticket-scheduled)+v1"; }
 
 int ts_create(ts_ctx** out, int N, const double* h, const double* J)
 {
@@ -207,7 +207,10 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->opt_l2_promotion = env_int("TS_L2_PROMOTION", 0);
     c->opt_max_ctas = 0;
     c->opt_l2_hints = env_int("TS_L2_HINTS", 1);
+    c->opt_pair = env_int("TS_PAIR", 1);
+    c->opt_probe = 0;
     c->d_chunk_ctr = nullptr; c->chunk_ctr_cap = 0;
+    c->d_sched = nullptr;
     c->d_energy[0] = c->d_energy[1] = c->d_energy[2] = nullptr;
     c->tmap_psi = nullptr;
     c->d_red = nullptr; c->red_cap = 0;
@@ -223,6 +226,8 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     if (e == cudaSuccess) e = cudaMalloc(&c->d_Jeff, sizeof(c->Jeff));
     if (e == cudaSuccess) e = cudaMemcpy(c->d_h, c->h, sizeof(c->h), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(c->d_Jeff, c->Jeff, sizeof(c->Jeff), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, 2 * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 2 * sizeof(unsigned int));   // kernels leave it at zero
     if (e == cudaSuccess) e = ts_tile_init();
     if (e == cudaSuccess) e = ts_small_init();
     if (e != cudaSuccess) { cudaGetLastError(); ts_destroy(c); return cuda_status(e); }
@@ -247,6 +252,7 @@ int ts_destroy(ts_ctx* c)
     ts_naive_free_stored(c);
     if (c->d_red) cudaFree(c->d_red);
     if (c->d_chunk_ctr) cudaFree(c->d_chunk_ctr);
+    if (c->d_sched) cudaFree(c->d_sched);
     if (c->d_trace) cudaFree(c->d_trace);
     for (auto& r : c->recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto& e : c->ev_pool) cudaEventDestroy(e);
@@ -349,12 +355,14 @@ int ts_set_option(ts_ctx* c, int key, int value)
 {
     if (!c) return TS_ERR_ARG;
     switch (key) {
-    case TS_OPT_KERNEL: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_kernel = value; break;
+    case TS_OPT_KERNEL: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_kernel = value; break;
     case TS_OPT_CHUNK: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_chunk = value; break;
     case TS_OPT_CHUNK_MAX_LOG2: if (value < TS_TILE_LOG2 + 1 || value > 26) return TS_ERR_ARG; c->opt_chunk_max_log2 = value; break;
     case TS_OPT_L2_PROMOTION: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_l2_promotion = value; c->tmaps.clear(); break;
     case TS_OPT_MAX_CTAS: if (value < 0) return TS_ERR_ARG; c->opt_max_ctas = value; break;
     case TS_OPT_L2_HINTS: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_l2_hints = value; break;
+    case TS_OPT_PAIR: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_pair = value; break;
+    case TS_OPT_PROBE: if (value < 0 || value > 3) return TS_ERR_ARG; c->opt_probe = value; break;
     case TS_OPT_DIAG_SOURCE:
         if (value < 0 || value > 1) return TS_ERR_ARG;
         c->opt_diag_source = value;
@@ -385,6 +393,8 @@ int ts_get_option(ts_ctx* c, int key, int* value)
     case TS_OPT_DIAG_SOURCE: *value = c->opt_diag_source; break;
     case TS_OPT_MAX_CTAS: *value = c->opt_max_ctas; break;
     case TS_OPT_L2_HINTS: *value = c->opt_l2_hints; break;
+    case TS_OPT_PAIR: *value = c->opt_pair; break;
+    case TS_OPT_PROBE: *value = c->opt_probe; break;
     default: return TS_ERR_ARG;
     }
     return TS_OK;
@@ -456,7 +466,7 @@ int ts_describe_plan(ts_ctx* c, char* buf, int buflen)
             else snprintf(tmp, sizeof tmp, " H[spins %d..%d, run 2^%d]", t.g0, t.g0 + TS_TILE_LOG2 - t.s - 1, t.s);
             s += tmp;
         }
-        snprintf(tmp, sizeof tmp, "; kernels=%s", c->opt_kernel == 2 ? "v3" : c->opt_kernel ? "v2" : "v1");
+        snprintf(tmp, sizeof tmp, "; kernels=%s", c->opt_kernel ? "v2" : "v1");
         s += tmp;
         if (ts_tile_chunk_supported(c, 1, SW_YDAG, SW_Y)) {
             const TileGroup& t = c->groups[1];

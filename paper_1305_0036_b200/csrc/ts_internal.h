@@ -82,6 +82,9 @@ struct ts_ctx {
     int opt_l2_promotion;                // tensor-map L2 promotion of the high groups: 0 none, 1 128 B, 2 256 B
     int opt_max_ctas;                    // upper bound on the persistent kernels' grid (0: one CTA per SM)
     int opt_l2_hints;                    // L2 eviction priorities on the TMA transfers of the L2-blocked launch
+    int opt_pair;                        // tickets of a high group are pairs of adjacent tiles
+    int opt_probe;                       // copy-only tile passes (the compute groups skip the tile body): pipeline ceilings
+    unsigned int* d_sched;               // [2] ticket counter + finished-CTA counter of the persistent kernels (zero between launches)
     unsigned int* d_chunk_ctr;           // done counters of the triple launch
     size_t chunk_ctr_cap;
     std::vector<TensorMapSlot> tmaps;    // per group, for the bound state pointer tmap_psi

@@ -8,15 +8,15 @@
 
 #include <mutex>
 
-#include "ts_tile_v3.cuh"
+#include "ts_tile_v2.cuh"
 
 namespace {
 
 tile_kernel_t g_tab[5][5];                 // k_tile_pass, run-time butterfly masks
 v2_kernel_t g_v2[3][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits
 v2_chunk_kernel_t g_v2_chunk[2][2];        // [9-bit high group][(Y^dag, Y), (X, X^dag)]
-v2_kernel_t g_v3[3][5][5];                 // the same for the 16-amplitudes-per-thread family (ts_tile_v3.cuh)
-v2_chunk_kernel_t g_v3_chunk[2][2];
+v2_chunk_kernel_t g_probe_chunk[2];        // measurement builds (ts_v2_probe.cu): [arithmetic only, exchanges only]
+v2_kernel_t g_probe_H[2], g_probe_A[2];
 PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
 std::once_flag g_once;
 cudaError_t g_init_status = cudaSuccess;
@@ -26,8 +26,8 @@ cudaError_t g_init_status = cudaSuccess;
 struct PhaseGeom {
     double t;
     int N, nfixed;
-    int nr, nt;          // register bits / thread bits at diagonal time (5 + 7, or 4 + 8 for the v3 kernels)
-    int rec;             // entries of a tile-phase record: 32 (nr = 5) or 40 (nr = 4)
+    int nr, nt;          // register bits / thread bits at diagonal time (5 + 7)
+    int rec;             // entries of a tile-phase record (32)
     int rspin[5], tspin[8], xspin[TS_MAX_FIXED];
 };
 
@@ -38,13 +38,12 @@ inline bool v2_geometry_ok(const TileGroup& g) { return g.is_low || (g.s >= 3 &&
 inline int nib(uint32_t pack, int i) { return (int)((pack >> (4 * i)) & 15u); }
 inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : 1); }     // kernel table index
 
-// layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2', H2 or H1).  layout 2: v3
-// (ts_tile_v3.cuh: A3, H2 or H1; four register bits, eight thread bits).
+// layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2', H2 or H1).
 PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
 {
     PhaseGeom q;
     q.t = t; q.N = c->N; q.nfixed = c->N - TS_TILE_LOG2;
-    q.nr = (layout == 2) ? 4 : 5; q.nt = TS_TILE_LOG2 - q.nr; q.rec = (layout == 2) ? TS_V3_REC : 32;
+    q.nr = 5; q.nt = TS_TILE_LOG2 - q.nr; q.rec = 32;
     for (int b = 0; b < 5; ++b) q.rspin[b] = 0;
     for (int b = 0; b < 8; ++b) q.tspin[b] = 0;
     const bool two = two_stage(g);
@@ -54,17 +53,11 @@ PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
             const int f = two ? (b < 2 ? b : 5 + b) : b;     // layout 2: thread bits 0,1 -> f 0,1; 2..6 -> f 7..11
             q.tspin[b] = spin_of_fbit(g, f);
         }
-    } else if (layout == 1) {
+    } else {
         const uint32_t RP = g.is_low ? TS_V2_A2S_R : (two ? TS_V2_H2_R : TS_V2_H1_R);
         const uint32_t TP = g.is_low ? TS_V2_A2S_T : (two ? TS_V2_H2_T : TS_V2_H1_T);
         for (int b = 0; b < 5; ++b) q.rspin[b] = spin_of_fbit(g, nib(RP, b));
         for (int b = 0; b < 7; ++b) q.tspin[b] = spin_of_fbit(g, nib(TP, b));
-    } else {
-        const bool two3 = !g.is_low && n_bfly(g) > 4;
-        const uint32_t RP = g.is_low ? TS_V3_A3_R : (two3 ? TS_V3_H2_R : TS_V3_H1_R);
-        const uint32_t TP = g.is_low ? TS_V3_A3_T : (two3 ? TS_V3_H2_T : TS_V3_H1_T);
-        for (int b = 0; b < 4; ++b) q.rspin[b] = spin_of_fbit(g, nib(RP, b));
-        for (int b = 0; b < 8; ++b) q.tspin[b] = spin_of_fbit(g, nib(TP, b));
     }
     bool in_tile[TS_MAX_N] = {false};
     for (int f = 0; f < TS_TILE_LOG2; ++f) in_tile[spin_of_fbit(g, f)] = true;
@@ -202,16 +195,7 @@ void init_once()
     ts_v2_register_chunk1(g_v2_chunk);
     ts_v2_register_chunk0_h9(g_v2_chunk);
     ts_v2_register_chunk1_h9(g_v2_chunk);
-    memset(g_v3, 0, sizeof(g_v3));
-    ts_v3_register_A(&g_v3[0]);
-    ts_v3_register_Hf(&g_v3[1]);
-    ts_v3_register_Hs(&g_v3[1]);
-    ts_v3_register_H9(&g_v3[2]);
-    memset(g_v3_chunk, 0, sizeof(g_v3_chunk));
-    ts_v3_register_chunk0(g_v3_chunk);
-    ts_v3_register_chunk1(g_v3_chunk);
-    ts_v3_register_chunk0_h9(g_v3_chunk);
-    ts_v3_register_chunk1_h9(g_v3_chunk);
+    ts_v2_register_probe(g_probe_chunk, g_probe_H, g_probe_A);
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
@@ -227,15 +211,11 @@ void init_once()
         for (int v = 0; v < 2 && e == cudaSuccess; ++v)
             if (g_v2_chunk[hm][v])
                 e = cudaFuncSetAttribute((const void*)g_v2_chunk[hm][v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
-    for (int ty = 0; ty < 3 && e == cudaSuccess; ++ty)
-        for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
-            for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
-                if (g_v3[ty][k1][k2])
-                    e = cudaFuncSetAttribute((const void*)g_v3[ty][k1][k2], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V3_SMEM);
-    for (int hm = 0; hm < 2 && e == cudaSuccess; ++hm)
-        for (int v = 0; v < 2 && e == cudaSuccess; ++v)
-            if (g_v3_chunk[hm][v])
-                e = cudaFuncSetAttribute((const void*)g_v3_chunk[hm][v], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V3_SMEM);
+    for (int m = 0; m < 2 && e == cudaSuccess; ++m) {
+        e = cudaFuncSetAttribute((const void*)g_probe_chunk[m], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)g_probe_H[m], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)g_probe_A[m], cudaFuncAttributeMaxDynamicSharedMemorySize, TS_V2_SMEM);
+    }
     for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
         for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
             if (g_tab[k1][k2])
@@ -267,18 +247,17 @@ void fill_v1_params(const ts_ctx* c, const TileGroup& g, const DiagTables* tb, T
     else { p->bf1 = 31u; p->bf2 = (31u << (10 - nb)) & 31u; }                       // top nb-5 bits of f 2..6
 }
 
-// family: 1 = v2 (32 amplitudes per thread), 2 = v3 (16)
-void fill_v2_geom(const TileGroup& g, int family, V2Geom* q)
+void fill_v2_geom(const TileGroup& g, V2Geom* q)
 {
     q->type = g.is_low ? 0 : 1;
     q->s = g.s; q->g0 = g.g0;
     q->m = g.is_low ? 0 : TS_TILE_LOG2 - g.s;
     q->nmid = g.g0 - g.s;
-    q->two_stage = (!g.is_low && q->m > (family == 2 ? 4 : 5)) ? 1 : 0;
+    q->two_stage = (!g.is_low && q->m > 5) ? 1 : 0;
     q->mask1 = 0u; q->mask2 = 0u;
     if (!g.is_low) {
-        q->mask1 = family == 2 ? v3_h_mask1(q->m) : tsk::v2_h_mask1(q->m);
-        q->mask2 = family == 2 ? v3_h_mask2(q->m) : tsk::v2_h_mask2(q->m);   // (v2: H2 register bit 4 = f 7 is a filler)
+        q->mask1 = tsk::v2_h_mask1(q->m);
+        q->mask2 = tsk::v2_h_mask2(q->m);   // (H2 register bit 4 = f 7 is a filler)
     }
 }
 
@@ -401,7 +380,6 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
 {
     const TileGroup& g = c->groups[group];
     if (c->opt_kernel == 0 || !v2_geometry_ok(g)) return 0;
-    if (c->opt_kernel == 2) return g_v3[v2_type(g)][kind1][kind2] ? 2 : 0;
     return g_v2[v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
@@ -418,17 +396,24 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
     const bool fused = (kind1 != SW_NONE && kind2 != SW_NONE);
     if (layout >= 1) {
         V2Pass p;
-        fill_v2_geom(g, layout, &p.g);
+        fill_v2_geom(g, &p.g);
         fill_v2_diag(tb, &p.d);
         p.ntiles = ntiles;
+        p.sched = c->d_sched;
+        p.pair_log2 = (c->opt_pair && !g.is_low && g.g0 > g.s && ntiles >= 2) ? 1u : 0u;   // adjacent tiles exist (nmid >= 1)
+        p.probe = (c->opt_probe == 1);
+        v2_kernel_t kern = g_v2[v2_type(g)][kind1][kind2];
+        if (c->opt_probe >= 2) {                       // measurement builds exist for the fused passes of the N = 30 plan
+            if (v2_type(g) == 2 && fused) kern = g_probe_H[c->opt_probe - 2];     // (the kinds do not change the cost)
+            if (v2_type(g) == 0 && fused) kern = g_probe_A[c->opt_probe - 2];
+        }
         CUtensorMap tm;
         cudaError_t e = v2_tensor_map(c, group, &tm);
         if (e != cudaSuccess) return e;
         const uint64_t cap = (c->opt_max_ctas > 0 && c->opt_max_ctas < c->num_sms) ? (uint64_t)c->opt_max_ctas : (uint64_t)c->num_sms;
         const uint64_t grid = ntiles < cap ? ntiles : cap;
         ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
-        if (layout == 2) g_v3[v2_type(g)][kind1][kind2]<<<(unsigned)grid, TS_V3_THREADS, TS_V3_SMEM, c->stream>>>(p, tm);
-        else g_v2[v2_type(g)][kind1][kind2]<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
+        kern<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
         ts_prof_end(c);
         return cudaGetLastError();
     }
@@ -452,7 +437,7 @@ bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
     if (C >= c->N || C > c->opt_chunk_max_log2) return false;          // at least two chunks, each small enough for L2
     const int v = (ka == SW_YDAG && kb == SW_Y) ? 0 : (ka == SW_X && kb == SW_XDAG) ? 1 : -1;
-    return v >= 0 && (c->opt_kernel == 2 ? g_v3_chunk : g_v2_chunk)[g.s == 3 ? 1 : 0][v] != nullptr;
+    return v >= 0 && g_v2_chunk[g.s == 3 ? 1 : 0][v] != nullptr;
 }
 
 cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int kb)
@@ -462,9 +447,8 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
     const uint32_t nchunks = 1u << (c->N - C);
     const DiagTables* tb = nullptr;
     cudaError_t e = cudaSuccess;
-    const int family = (c->opt_kernel == 2) ? 2 : 1;
     if (d.present) {
-        e = ts_tile_get_tables(c, d, 0, family, &tb);
+        e = ts_tile_get_tables(c, d, 0, 1, &tb);
         if (e != cudaSuccess) return e;
     }
     const size_t nctr = 2 * (size_t)nchunks;
@@ -478,10 +462,12 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
         c->chunk_ctr_cap = nctr;
     }
     V2Chunk q;
-    fill_v2_geom(g, family, &q.gh);
-    fill_v2_geom(c->groups[0], family, &q.ga);
+    fill_v2_geom(g, &q.gh);
+    fill_v2_geom(c->groups[0], &q.ga);
     fill_v2_diag(tb, &q.d);
     q.done = c->d_chunk_ctr;
+    q.sched = c->d_sched;
+    q.probe = (c->opt_probe == 1);
     q.nchunks = nchunks; q.tiles_log2 = (uint32_t)(C - TS_TILE_LOG2);
     q.l2_hints = c->opt_l2_hints;
     e = cudaMemsetAsync(c->d_chunk_ctr, 0, sizeof(unsigned int) * nctr, c->stream);
@@ -497,12 +483,9 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
     ts_prof_begin(c, TS_KC_TILE_CHUNK, 3.0);
     // cooperative launch: the loaders wait on other CTAs' progress, so all CTAs must be resident (else: error, not a hang)
     void* args[3] = {(void*)&q, (void*)&tmA, (void*)&tmH};
-    if (family == 2)
-        e = cudaLaunchCooperativeKernel((const void*)g_v3_chunk[g.s == 3 ? 1 : 0][v], dim3((unsigned)grid), dim3(TS_V3_THREADS), args,
-                                        TS_V3_SMEM, c->stream);
-    else
-        e = cudaLaunchCooperativeKernel((const void*)g_v2_chunk[g.s == 3 ? 1 : 0][v], dim3((unsigned)grid), dim3(TS_V2_THREADS), args,
-                                        TS_V2_SMEM, c->stream);
+    const void* kern = (const void*)g_v2_chunk[g.s == 3 ? 1 : 0][v];
+    if (c->opt_probe >= 2 && g.s == 3) kern = (const void*)g_probe_chunk[c->opt_probe - 2];
+    e = cudaLaunchCooperativeKernel(kern, dim3((unsigned)grid), dim3(TS_V2_THREADS), args, TS_V2_SMEM, c->stream);
     ts_prof_end(c);
     return e;
 }

@@ -16,6 +16,13 @@
 //     for rows of 8 amplitudes (128 B).  All register layouts below keep one of {f0|f3}, {f1|f4}, {f2|f5} on each of
 //     the three low lane bits, which makes every 128-bit shared-memory access conflict-free under that swizzle.
 //
+//   * tiles are handed out DYNAMICALLY: the loader draws tickets from a global counter (one atomicAdd per ticket, fetched
+//     one ticket ahead) and passes the tile index to the compute groups and the storer through a shared-memory slot per
+//     buffer.  SMs do not run at the same speed (ncu, static assignment: fastest SM done after 5.6 ms, slowest after
+//     7.9 ms of a 7.9 ms top-group pass, profiles/r02a_baseline.md), so a static split leaves a fifth of the chip idle at
+//     the end of every pass.  A ticket of a high group is a PAIR of adjacent tiles (2p, 2p + 1): their 128-byte rows are
+//     the two halves of 256-byte segments.
+//
 // In-tile index f (12 bits): group A (spins 0..11): f = spin.  High group (s run bits, m = 12 - s group bits):
 // f < s <-> spin f, f >= s <-> spin g0 + f - s; the tile is 2^m rows of 2^s amplitudes at a stride of 2^g0.
 //
@@ -37,7 +44,9 @@
 #define TS_V2_NBUF 3
 #define TS_V2_TILE_BYTES 65536
 #define TS_V2_OFF_TP (TS_V2_NBUF * TS_V2_TILE_BYTES)         // 3 x 512 B tile-phase records
-#define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3], tab mbarriers
+#define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3], tab mbarriers (80 B), then tile[3] (u32)
+#define TS_V2_OFF_TILE (TS_V2_OFF_BAR + 96)                  // tile index of the job in each buffer (written by the loader)
+#define TS_V2_END 0xffffffffu                                // "no more tiles" marker in a tile slot
 #define TS_V2_OFF_TAB (TS_V2_OFF_BAR + 128)                  // per-launch phase tables: TT[128], WT[5][128], RR[32]
 #define TS_V2_TAB_BYTES (800 * 16)
 #define TS_V2_SMEM (TS_V2_OFF_TAB + TS_V2_TAB_BYTES)
@@ -77,6 +86,9 @@ struct V2Pass {
     V2Geom g;
     V2Diag d;
     uint64_t ntiles;
+    unsigned int* sched;         // [2]: next ticket, CTAs finished (both zero between launches: the last CTA resets them)
+    uint32_t pair_log2;          // tiles per ticket = 2^pair_log2 (1: adjacent tile pairs of a high group)
+    int probe;                   // 1: copy only -- the compute groups skip the tile body (TS_OPT_PROBE: pipeline ceilings)
 };
 
 // L2-blocked triple launch: [high group, sweep KA] [group A: KA . D . KB] [high group, sweep KB] chunk by chunk.
@@ -84,7 +96,9 @@ struct V2Chunk {
     V2Geom gh, ga;
     V2Diag d;
     unsigned int* done;          // [2][nchunks] tiles finished (and globally visible) of phase 1 / phase 2 of a chunk
+    unsigned int* sched;         // [2]: next ticket, CTAs finished
     uint32_t nchunks, tiles_log2;
+    int probe;
     int l2_hints;                // 1: eviction priorities on the TMA transfers (keep a chunk in L2 until its third phase wrote it)
 };
 
@@ -103,6 +117,10 @@ void ts_v2_register_chunk0(v2_chunk_kernel_t (*tab)[2]);
 void ts_v2_register_chunk1(v2_chunk_kernel_t (*tab)[2]);
 void ts_v2_register_chunk0_h9(v2_chunk_kernel_t (*tab)[2]);
 void ts_v2_register_chunk1_h9(v2_chunk_kernel_t (*tab)[2]);
+// measurement builds of the N = 30 kernels (ts_v2_probe.cu): mode 1 = arithmetic only (no layout exchanges), 2 = exchanges
+// only (no arithmetic); index [mode - 1].  chunk: (Y^dag, Y) with a 9-bit high group; fusedH: top group (X^dag, Y^dag);
+// fusedA: group A (Y^dag, Y)
+void ts_v2_register_probe(v2_chunk_kernel_t* chunk, v2_kernel_t* fusedH, v2_kernel_t* fusedA);
 
 #ifdef __CUDACC__
 namespace tsk {
@@ -305,10 +323,12 @@ __device__ __forceinline__ void v2_apply_diag(const double2* RR, const double2 b
 // ------------------------------------------------------------------------------------------------ tile bodies
 // The tile is in `buf` (landed by TMA); on return the finished tile is in `buf` again, in the same slots.
 // diag: apply the diagonal; tp: this tile's phase record; tab: the launch's thread tables (both in shared memory).
-template <int K1, int K2>
+// MODE (measurement builds, ts_v2_probe.cu): bit 0 = do the arithmetic, bit 1 = do the layout exchanges; 3 = the product.
+template <int K1, int K2, int MODE = 3>
 __device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, const double scale, const double2* tp,
                                           const double2* tab, const int t, const int grp)
 {
+    constexpr bool AR = (MODE & 1) != 0, EX = (MODE & 2) != 0;
     using L1 = V2Layout<TS_V2_A1_R, TS_V2_A1_T>;
     using L2 = V2Layout<TS_V2_A2_R, TS_V2_A2_T>;
     using L1S = V2Layout<TS_V2_A1S_R, TS_V2_A1S_T>;
@@ -317,34 +337,45 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, c
     double re[32], im[32];
     if (K1 != SW_NONE) {
         L1::load(buf, o1, re, im);
-        bfly_regs<K1, 31>(re, im, 0u);                 // f 3,4,5,10,11
-        L1::store(buf, o1, re, im);
-        v2_group_sync(grp);
-        L2::load(buf, o2, re, im);
-        bfly_regs<K1, 31>(re, im, 0u);                 // f 0,1,2,8,9
-        L2::store(buf, o2, re, im);                    // A2 -> A2': lanes <-> registers inside the warp's own quarter
-        __syncwarp();
+        if (AR) bfly_regs<K1, 31>(re, im, 0u);         // f 3,4,5,10,11
+        if (EX) {
+            L1::store(buf, o1, re, im);
+            v2_group_sync(grp);
+            L2::load(buf, o2, re, im);
+        }
+        if (AR) bfly_regs<K1, 31>(re, im, 0u);         // f 0,1,2,8,9
+        if (EX) {
+            L2::store(buf, o2, re, im);                // A2 -> A2': lanes <-> registers inside the warp's own quarter
+            __syncwarp();
+        }
     }
-    L2S::load(buf, o2s, re, im);
-    bfly_regs<K1, 24>(re, im, 0u);                     // f 6,7
-    if (diag) {
+    if (EX || K1 == SW_NONE) L2S::load(buf, o2s, re, im);
+    if (AR) bfly_regs<K1, 24>(re, im, 0u);             // f 6,7
+    if (diag && AR) {
         double2 base, w[5];
         v2_thread_phase(scale, tp, tab, t, base, w);
         v2_apply_diag(tab + 768, base, w, re, im);
     }
     if (K2 != SW_NONE) {
-        bfly_regs<K2, 31>(re, im, 0u);                 // f 0,1,2,6,7
-        L2S::store(buf, o2s, re, im);
-        v2_group_sync(grp);
-        L1::load(buf, o1, re, im);
-        bfly_regs<K2, 31>(re, im, 0u);                 // f 3,4,5,10,11
-        L1::store(buf, o1, re, im);                    // A1 -> A1'
-        __syncwarp();
-        L1S::load(buf, o1s, re, im);
-        bfly_regs<K2, 24>(re, im, 0u);                 // f 8,9
-        L1S::store(buf, o1s, re, im);
+        if (AR) bfly_regs<K2, 31>(re, im, 0u);         // f 0,1,2,6,7
+        if (EX) {
+            L2S::store(buf, o2s, re, im);
+            v2_group_sync(grp);
+            L1::load(buf, o1, re, im);
+        }
+        if (AR) bfly_regs<K2, 31>(re, im, 0u);         // f 3,4,5,10,11
+        if (EX) {
+            L1::store(buf, o1, re, im);                // A1 -> A1'
+            __syncwarp();
+            L1S::load(buf, o1s, re, im);
+        }
+        if (AR) bfly_regs<K2, 24>(re, im, 0u);         // f 8,9
+        if (EX) L1S::store(buf, o1s, re, im);
+        else if (K1 != SW_NONE) L1::store(buf, o1, re, im);
+        else L2S::store(buf, o2s, re, im);
     } else {
-        L2S::store(buf, o2s, re, im);
+        if (EX) L2S::store(buf, o2s, re, im);
+        else L1::store(buf, o1, re, im);
     }
 }
 
@@ -355,39 +386,40 @@ __host__ __device__ constexpr unsigned v2_h_mask2(int m) { unsigned k = 0; for (
 
 // M > 0: the number of group bits is a compile-time constant (masks folded: no run-time branches around the butterfly
 // levels); M = -1: taken from g at run time.
-template <int K1, int K2, int M>
+template <int K1, int K2, int M, int MODE = 3>
 __device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, const bool diag, const double scale, const double2* tp,
                                           const double2* tab, const int t, const int grp)
 {
+    constexpr bool AR = (MODE & 1) != 0, EX = (MODE & 2) != 0;
     using L1 = V2Layout<TS_V2_H1_R, TS_V2_H1_T>;
     using L2 = V2Layout<TS_V2_H2_R, TS_V2_H2_T>;
     constexpr bool CT = (M > 0);
     constexpr int MK1 = CT ? (int)v2_h_mask1(M > 0 ? M : 1) : -1;
     constexpr int MK2 = CT ? (int)v2_h_mask2(M > 0 ? M : 1) : -1;
     const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t);
-    const bool two = CT ? (M > 5) : (g.two_stage != 0);
+    const bool two = EX && (CT ? (M > 5) : (g.two_stage != 0));
     double re[32], im[32];
     L1::load(buf, o1, re, im);
-    bfly_regs<K1, MK1>(re, im, g.mask1);
+    if (AR) bfly_regs<K1, MK1>(re, im, g.mask1);
     if (two) {
         L1::store(buf, o1, re, im);
         v2_group_sync(grp);
         L2::load(buf, o2, re, im);
-        bfly_regs<K1, MK2>(re, im, g.mask2);
     }
-    if (diag) {
+    if (AR && (two || !EX)) bfly_regs<K1, MK2>(re, im, g.mask2);
+    if (diag && AR) {
         double2 base, w[5];
         v2_thread_phase(scale, tp, tab, t, base, w);
         v2_apply_diag(tab + 768, base, w, re, im);
     }
     if (K2 != SW_NONE) {
+        if (AR && (two || !EX)) bfly_regs<K2, MK2>(re, im, g.mask2);
         if (two) {
-            bfly_regs<K2, MK2>(re, im, g.mask2);
             L2::store(buf, o2, re, im);
             v2_group_sync(grp);
             L1::load(buf, o1, re, im);
         }
-        bfly_regs<K2, MK1>(re, im, g.mask1);
+        if (AR) bfly_regs<K2, MK1>(re, im, g.mask1);
         L1::store(buf, o1, re, im);
     } else {
         if (two) L2::store(buf, o2, re, im);
@@ -485,9 +517,43 @@ __device__ __forceinline__ void v2_init_barriers(const uint32_t sBar)
     v2_fence_async_smem();
 }
 
+// ------------------------------------------------------------------------------------------------ scheduling
+// Tickets.  sched[0] is the next ticket; the loader (one lane) draws them with atomicAdd, always one ahead of the ticket
+// it is loading so that the atomic's round trip to L2 is never on its critical path.  sched[1] counts CTAs whose loader is
+// done; the last one sets both words back to zero, so every launch starts from 0 without a memset in between.
+__device__ __forceinline__ uint32_t v2_ticket_next(unsigned int* sched) { return atomicAdd(sched, 1u); }
+__device__ __forceinline__ void v2_ticket_finish(unsigned int* sched)
+{
+    __threadfence();
+    if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) {      // every other CTA has drawn its last ticket already
+        sched[0] = 0u;
+        sched[1] = 0u;
+        __threadfence();
+    }
+}
+__device__ __forceinline__ uint32_t v2_ld_tile(const unsigned char* smraw, uint32_t b)
+{
+    return *reinterpret_cast<const volatile uint32_t*>(smraw + TS_V2_OFF_TILE + 4u * b);
+}
+__device__ __forceinline__ void v2_st_tile(unsigned char* smraw, uint32_t b, uint32_t v)
+{
+    *reinterpret_cast<volatile uint32_t*>(smraw + TS_V2_OFF_TILE + 4u * b) = v;
+}
+// The loader's epilogue: two END markers, one for each compute group (local jobs j and j + 1 belong to different groups;
+// the storer leaves at the first).  A marker completes the buffer's `full` phase with a plain arrive (no bytes expected).
+__device__ __forceinline__ void v2_push_end(unsigned char* smraw, const uint32_t sBar, uint64_t j)
+{
+    for (int k = 0; k < 2; ++k, ++j) {
+        const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+        if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
+        v2_st_tile(smraw, b, TS_V2_END);
+        v2_mbar_arrive(sBar + 8 * b);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ one tile pass
-// TYPE 0: group A, 1: high group (any m), 2: high group with m = 9 (masks folded).  CTA b runs tiles b, b + G, ...
-template <int TYPE, int K1, int K2>
+// TYPE 0: group A, 1: high group (any m), 2: high group with m = 9 (masks folded).  MODE: see v2_body_A.
+template <int TYPE, int K1, int K2, int MODE = 3>
 __global__ void __launch_bounds__(TS_V2_THREADS, 1)
 k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap tmap)
 {
@@ -495,8 +561,6 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
     const uint32_t sBase = v2_smem_u32(smraw);
     const uint32_t sBar = sBase + TS_V2_OFF_BAR;
     const int warp = threadIdx.x >> 5;
-    const uint64_t G = gridDim.x;
-    const uint64_t n_cta = (p.ntiles > blockIdx.x) ? (p.ntiles - blockIdx.x + G - 1) / G : 0;
     const bool has_diag = (p.d.tile_phase != nullptr);
 
     if (threadIdx.x == 0) {
@@ -512,20 +576,33 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
                 v2_mbar_expect_tx(sBar + 8 * 3 * TS_V2_NBUF, TS_V2_TAB_BYTES);
                 v2_bulk_load(sBase + TS_V2_OFF_TAB, p.d.tables, TS_V2_TAB_BYTES, sBar + 8 * 3 * TS_V2_NBUF);
             }
-            for (uint64_t j = 0; j < n_cta; ++j) {
-                const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-                if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
-                const uint64_t tile = blockIdx.x + j * G;
-                const uint32_t bar = sBar + 8 * b;
-                v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (has_diag ? 512u : 0u));
-                if (has_diag) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, p.d.tile_phase + (tile << 5), 512u, bar);
-                v2_issue_load(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+            const uint32_t per = 1u << p.pair_log2;
+            const uint64_t ntick = p.ntiles >> p.pair_log2;
+            uint64_t j = 0;
+            uint32_t tk = v2_ticket_next(p.sched);
+            while (tk < ntick) {
+                const uint32_t nxt = v2_ticket_next(p.sched);
+                for (uint32_t u = 0; u < per; ++u, ++j) {
+                    const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
+                    if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
+                    const uint64_t tile = ((uint64_t)tk << p.pair_log2) + u;
+                    const uint32_t bar = sBar + 8 * b;
+                    v2_st_tile(smraw, b, (uint32_t)tile);
+                    v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (has_diag ? 512u : 0u));
+                    if (has_diag) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, p.d.tile_phase + (tile << 5), 512u, bar);
+                    v2_issue_load(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+                }
+                tk = nxt;
             }
+            v2_push_end(smraw, sBar, j);
+            v2_ticket_finish(p.sched);
         } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
-            for (uint64_t j = 0; j < n_cta; ++j) {
+            for (uint64_t j = 0;; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
                 v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
-                v2_issue_store(p.g, &tmap, blockIdx.x + j * G, sBase + b * TS_V2_TILE_BYTES);
+                const uint32_t tile = v2_ld_tile(smraw, b);
+                if (tile == TS_V2_END) break;
+                v2_issue_store(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES);
                 v2_store_commit();
                 v2_store_wait_read();
                 v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
@@ -539,16 +616,20 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
         const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
         const double scale = p.d.scale;
         if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
-        for (uint64_t j = grp; j < n_cta; j += 2) {
+        for (uint64_t j = grp;; j += 2) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
             v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
-            unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
-            const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
-            if constexpr (TYPE == 0) v2_body_A<K1, K2>(buf, has_diag, scale, tp, tab, t, grp);
-            else if constexpr (TYPE == 2) v2_body_H<K1, K2, 9>(buf, p.g, has_diag, scale, tp, tab, t, grp);
-            else v2_body_H<K1, K2, -1>(buf, p.g, has_diag, scale, tp, tab, t, grp);
-            v2_fence_async_smem();                     // my shared-memory writes -> visible to the TMA store
+            const bool end = (v2_ld_tile(smraw, b) == TS_V2_END);
+            if (!end && !p.probe) {
+                unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
+                const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
+                if constexpr (TYPE == 0) v2_body_A<K1, K2, MODE>(buf, has_diag, scale, tp, tab, t, grp);
+                else if constexpr (TYPE == 2) v2_body_H<K1, K2, 9, MODE>(buf, p.g, has_diag, scale, tp, tab, t, grp);
+                else v2_body_H<K1, K2, -1, MODE>(buf, p.g, has_diag, scale, tp, tab, t, grp);
+                v2_fence_async_smem();                 // my shared-memory writes -> visible to the TMA store
+            }
             v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
+            if (end) break;
         }
     }
 }
@@ -559,13 +640,13 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
 // P1 = high group, sweep KA (from HBM);  P2 = group A, KA . D . KB (from L2);  P3 = high group, sweep KB (from L2, then
 // out to HBM).  A chunk is closed under all three (closed-set argument of P:141 applied to spins 0 .. C-1), so two
 // chunks (64 MiB) live in the 126 MB L2 at any time and the state makes ONE HBM round trip for three tile passes.
-// CTA b runs jobs b, b + G, ... ; a job of phase 2 / 3 may be LOADED once all T tiles of the previous phase of its chunk
-// are stored and visible: the loader polls done[phase - 1][chunk] (acquire) before it issues the TMA load, the storer
-// publishes a tile (release) once its TMA store has completed.  Only the loader ever waits on other CTAs, the compute
-// groups and the storer keep draining the jobs already loaded, and jobs are issued in increasing n on every CTA: the
-// smallest unfinished job never depends on an unfinished one, so the launch cannot deadlock as long as all CTAs are
-// resident (cooperative launch).
-template <int KA, int KB, int HM>
+// Job n is ticket n: tickets are drawn in increasing order and every CTA loads its tickets in the order it drew them.  A
+// job of phase 2 / 3 may be LOADED once all T tiles of the previous phase of its chunk are stored and visible: the loader
+// polls done[phase - 1][chunk] (acquire) before it issues the TMA load, the storer publishes a tile (release) once its TMA
+// store has completed.  Only the loader ever waits on other CTAs; the compute groups and the storer keep draining the
+// jobs already loaded.  The smallest unfinished ticket depends only on smaller tickets, all finished, and it is the
+// oldest job of the CTA that drew it: the launch cannot deadlock as long as all CTAs are resident (cooperative launch).
+template <int KA, int KB, int HM, int MODE = 3>
 __global__ void __launch_bounds__(TS_V2_THREADS, 1)
 k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmH)
 {
@@ -575,14 +656,11 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
     const int warp = threadIdx.x >> 5;
     const uint32_t tl = q.tiles_log2, T = 1u << tl;
     const uint32_t nblocks = 3u * q.nchunks;
-    const uint64_t total = (uint64_t)nblocks << tl;
-    const uint64_t G = gridDim.x;
-    const uint64_t n_cta = (total > blockIdx.x) ? (total - blockIdx.x + G - 1) / G : 0;
+    const uint32_t total = nblocks << tl;
     const bool has_diag = (q.d.tile_phase != nullptr);
 
-    auto job_of = [&](const uint64_t j, uint32_t& phase, uint32_t& c, uint64_t& tile) {
-        const uint64_t n = blockIdx.x + j * G;
-        const uint32_t B = (uint32_t)(n >> tl);
+    auto job_of = [&](const uint32_t n, uint32_t& phase, uint32_t& c, uint64_t& tile) {
+        const uint32_t B = n >> tl;
         if (B == nblocks - 1) { phase = 2; c = q.nchunks - 1; }
         else if (B < 5) { phase = (B < 2) ? 0u : (B < 4 ? 1u : 2u); c = (B == 1 || B == 3) ? 1u : 0u; }
         else {
@@ -610,10 +688,13 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
             // write is read again from L2 (evict last); the third phase's reads are the last use of a line.
             const uint64_t pol_ld[3] = {v2_policy(q.l2_hints ? 1 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
             uint32_t ok_key = 0xffffffffu;             // (phase, chunk) whose dependency was last seen satisfied
-            for (uint64_t j = 0; j < n_cta; ++j) {
+            uint64_t j = 0;
+            uint32_t n = v2_ticket_next(q.sched);
+            while (n < total) {
+                const uint32_t nxt = v2_ticket_next(q.sched);
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
                 uint32_t phase, c; uint64_t tile;
-                job_of(j, phase, c, tile);
+                job_of(n, phase, c, tile);
                 if (phase != 0) {
                     const uint32_t key = (phase << 28) | c;
                     if (key != ok_key) {
@@ -626,18 +707,25 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
                 if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
                 const uint32_t bar = sBar + 8 * b;
                 const bool tpl = has_diag && phase == 1;
+                v2_st_tile(smraw, b, n);
                 v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (tpl ? 512u : 0u));
                 if (tpl) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, q.d.tile_phase + (tile << 5), 512u, bar);
                 if (phase == 1) v2_issue_load_h(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[1]);
                 else v2_issue_load_h(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[phase]);
+                ++j;
+                n = nxt;
             }
+            v2_push_end(smraw, sBar, j);
+            v2_ticket_finish(q.sched);
         } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
             const uint64_t pol_st[3] = {v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
-            for (uint64_t j = 0; j < n_cta; ++j) {
+            for (uint64_t j = 0;; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-                uint32_t phase, c; uint64_t tile;
-                job_of(j, phase, c, tile);
                 v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
+                const uint32_t n = v2_ld_tile(smraw, b);
+                if (n == TS_V2_END) break;
+                uint32_t phase, c; uint64_t tile;
+                job_of(n, phase, c, tile);
                 if (phase == 1) v2_issue_store_h(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[1]);
                 else v2_issue_store_h(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[phase]);
                 v2_store_commit();
@@ -661,18 +749,27 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
         const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
         const double scale = q.d.scale;
         if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
-        for (uint64_t j = grp; j < n_cta; j += 2) {
+        for (uint64_t j = grp;; j += 2) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-            uint32_t phase, c; uint64_t tile;
-            job_of(j, phase, c, tile);
             v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
-            unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
-            const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
-            if (phase == 0) v2_body_H<KA, SW_NONE, HM>(buf, q.gh, false, 1.0, tp, tab, t, grp);
-            else if (phase == 1) v2_body_A<KA, KB>(buf, has_diag, scale, tp, tab, t, grp);
-            else v2_body_H<KB, SW_NONE, HM>(buf, q.gh, false, 1.0, tp, tab, t, grp);
-            v2_fence_async_smem();
+            const uint32_t n = v2_ld_tile(smraw, b);
+            const bool end = (n == TS_V2_END);
+            if (!end && !q.probe) {
+                const uint32_t B = n >> tl;
+                // phase of block B (see job_of): 0 / 2 = high group, 1 = group A
+                uint32_t phase;
+                if (B == nblocks - 1) phase = 2;
+                else if (B < 5) phase = (B < 2) ? 0u : (B < 4 ? 1u : 2u);
+                else { const uint32_t r = (B - 5) % 3; phase = (r == 0) ? 0u : (r == 1 ? 2u : 1u); }
+                unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
+                const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
+                if (phase == 0) v2_body_H<KA, SW_NONE, HM, MODE>(buf, q.gh, false, 1.0, tp, tab, t, grp);
+                else if (phase == 1) v2_body_A<KA, KB, MODE>(buf, has_diag, scale, tp, tab, t, grp);
+                else v2_body_H<KB, SW_NONE, HM, MODE>(buf, q.gh, false, 1.0, tp, tab, t, grp);
+                v2_fence_async_smem();
+            }
             v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
+            if (end) break;
         }
     }
 }

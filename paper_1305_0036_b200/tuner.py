@@ -4,7 +4,7 @@ The paper: "we developed a small tool that does a brute force search for the fas
 configuration for each number of spins is stored in a file and read at the start of the simulation".  Here the
 search space is what the C ABI exposes: the split of the N - 12 high index bits into groups (`ts_set_plan_groups`: how
 many bits each tile pass butterflies, hence run lengths and passes per sweep), whether the group above A is run as an
-L2-blocked triple launch (`TS_OPT_CHUNK`), and the kernel family (`TS_OPT_KERNEL`: 32 or 16 amplitudes per thread).  Every candidate is
+L2-blocked triple launch (`TS_OPT_CHUNK`), and the kernel family (`TS_OPT_KERNEL`).  Every candidate is
 timed on the device with CUDA events (median of `repeats` runs of `steps` 4th-order steps on a random state; throughput
 does not depend on the values), and the winner per N is written as one line of a plan file that `ts_load_plan_file` /
 the `TS_PLAN_FILE` environment variable read back.
@@ -57,7 +57,7 @@ def candidates(N: int, max_groups: int = 4, max_splits: int = 12) -> List[dict]:
     for groups in comps:
         chunk_possible = len(groups) >= 2 and 12 + groups[0] <= 21
         for chunk in ((1, 0) if chunk_possible else (0,)):
-            for kernel in (1, 2):        # 32 / 16 amplitudes per thread (ts_tile_v2.cuh / ts_tile_v3.cuh)
+            for kernel in (1,):          # the warp-specialised TMA kernels (ts_tile_v2.cuh)
                 out.append({"groups": list(groups), "chunk": chunk, "l2_promotion": 0, "kernel": kernel})
     return out
 

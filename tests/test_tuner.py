@@ -24,7 +24,7 @@ def test_candidates_put_the_default_plan_first_and_stay_bounded():
         assert all(sum(p["groups"]) == N - 12 for p in c)
         assert all(p["chunk"] == 0 or (len(p["groups"]) >= 2 and 12 + p["groups"][0] <= 21) for p in c)
     assert T.candidates(30)[0]["groups"] == [9, 9] and T.candidates(30)[0]["chunk"] == 1 and T.candidates(30)[0]["kernel"] == 1
-    assert {p["kernel"] for p in T.candidates(30)} == {1, 2}
+    assert {p["kernel"] for p in T.candidates(30)} == {1}
     assert T.candidates(27)[0]["groups"] == [9, 6]
 
 
