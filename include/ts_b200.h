@@ -202,6 +202,35 @@ const char* ts_strerror(int status);
 /* Library build info: "ts_b200 <version> sm_100a ..." */
 const char* ts_version(void);
 
+/* ---- one state vector sharded over 2^g GPUs (SURVEY 8 e, 8 f NEXT-5; beyond the paper, whose limit was device memory).
+ * Rank `rank` holds the 2^(N-g) amplitudes whose top g index bits equal `rank`; once per sweep the ranks swap the g rank
+ * bits with the top g local bits (an all-to-all; see csrc/ts_shard.cu for the two spin layouts and the effective local
+ * Hamiltonian of a shard).  The shard object owns two ordinary contexts, one per spin layout.
+ *   ts_shard_create   h [3][N], J [3][N][N] of the FULL system (copied); log2_ranks = g in 0..8, 2g <= N, N - g <= 33.
+ *   ts_shard_bind     two DEVICE buffers of 2^(N-g) complex128 each (caller-owned): the shard's amplitudes are in buf0, in
+ *                     layout 0 (local index = low N-g bits of the global index); buf1 is the exchange target.
+ *   ts_shard_evolve   psi <- U_order(tau)^n psi, collectively: EVERY rank must make the same call.  `exchange(user, src,
+ *                     dst)` must perform the index-bit swap of this rank's 2^(N-g) amplitudes from device buffer src to
+ *                     device buffer dst (block rho' of src, 2^(N-2g) amplitudes, goes to rank rho'; block rho' of dst
+ *                     receives from rank rho') on the shard's stream or ordered with it, and return 0; it is called 20
+ *                     times per 4th-order step (4 per 2nd-order step), an even number, so after the call the amplitudes
+ *                     are again in layout 0 and in the buffer they started in.  g = 0: exchange may be NULL.
+ *   ts_shard_info     local spin count, current layout (0 / 1) and current buffer (0 / 1).
+ *   ts_shard_spin_map spin_of_bit[N]: the spin on each local bit (first N-g entries), then on each rank bit, in `config`.
+ *   ts_shard_ctx      the context of a layout: for the read-only calls (ts_expect_all, ts_norm2, ts_get_state) on this
+ *                     rank's amplitudes; sums over ranks are the caller's (an all-reduce).  Do not evolve it directly.
+ * Errors: TS_ERR_ARG, TS_ERR_NOMEM, TS_ERR_CUDA (also when the callback fails), TS_ERR_NOSTATE (nothing bound). */
+typedef struct ts_shard ts_shard;
+typedef int (*ts_exchange_fn)(void* user, void* src_dev, void* dst_dev);
+int ts_shard_create(ts_shard** out, int N, const double* h, const double* J, int log2_ranks, int rank);
+int ts_shard_destroy(ts_shard* s);
+int ts_shard_bind(ts_shard* s, void* buf0_dev, void* buf1_dev);
+int ts_shard_set_stream(ts_shard* s, void* cuda_stream);
+int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exchange_fn exchange, void* user);
+int ts_shard_info(ts_shard* s, int* n_local, int* config, int* buffer);
+int ts_shard_spin_map(ts_shard* s, int config, int* spin_of_bit /*[N]*/);
+ts_ctx* ts_shard_ctx(ts_shard* s, int config);
+
 #ifdef __cplusplus
 }
 #endif

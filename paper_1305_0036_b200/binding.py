@@ -27,10 +27,13 @@ SYMBOLS = ("ts_create", "ts_destroy", "ts_set_stream", "ts_bind_state", "ts_set_
            "ts_set_state_range", "ts_get_state", "ts_evolve", "ts_evolve_observe", "ts_expect", "ts_expect_all", "ts_norm2", "ts_overlap", "ts_set_plan",
            "ts_describe_plan", "ts_set_profiling", "ts_get_profile", "ts_reset_profile", "ts_strerror", "ts_version",
            "ts_set_plan_groups", "ts_set_option", "ts_get_option", "ts_get_profile_passes", "ts_correlate", "ts_total_sz",
-           "ts_energy", "ts_set_random_phase_state", "ts_loschmidt_echo", "ts_load_plan_file")
+           "ts_energy", "ts_set_random_phase_state", "ts_loschmidt_echo", "ts_load_plan_file",
+           "ts_shard_create", "ts_shard_destroy", "ts_shard_bind", "ts_shard_set_stream", "ts_shard_evolve", "ts_shard_info",
+           "ts_shard_spin_map", "ts_shard_ctx")
 
 _lib = None
 _vp, _dp, _i64p = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)
+EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)   # ts_exchange_fn
 
 
 class TSError(RuntimeError):
@@ -79,6 +82,14 @@ def load() -> ctypes.CDLL:
         "ts_set_profiling": (I, [_vp, I]),
         "ts_get_profile": (I, [_vp, _i64p, _dp]),
         "ts_reset_profile": (I, [_vp]),
+        "ts_shard_create": (I, [ctypes.POINTER(_vp), I, _dp, _dp, I, I]),
+        "ts_shard_destroy": (I, [_vp]),
+        "ts_shard_bind": (I, [_vp, _vp, _vp]),
+        "ts_shard_set_stream": (I, [_vp, _vp]),
+        "ts_shard_evolve": (I, [_vp, D, I64, I, EXCHANGE_FN, _vp]),
+        "ts_shard_info": (I, [_vp, ctypes.POINTER(I), ctypes.POINTER(I), ctypes.POINTER(I)]),
+        "ts_shard_spin_map": (I, [_vp, I, ctypes.POINTER(I)]),
+        "ts_shard_ctx": (_vp, [_vp, I]),
         "ts_strerror": (ctypes.c_char_p, [I]),
         "ts_version": (ctypes.c_char_p, []),
     }

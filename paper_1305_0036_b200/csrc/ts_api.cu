@@ -189,6 +189,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->stream = 0;
     memset(c->h, 0, sizeof(c->h));
     memset(c->Jeff, 0, sizeof(c->Jeff));
+    c->e0[0] = c->e0[1] = c->e0[2] = 0.0;
     for (int a = 0; a < 3; ++a) {
         for (int j = 0; j < N; ++j) c->h[a][j] = h[a * N + j];
         for (int j = 0; j < N; ++j)
@@ -660,11 +661,11 @@ int ts_total_sz(ts_ctx* c, double* out)
     return TS_OK;
 }
 
-namespace {
+} // extern "C"
 
 // One global rotation (sweep) of the state, optionally followed by the exact scaling 2^scale_pow: every group of the
 // plan once (tiled), or one launch per spin (naive / small-N contexts).
-cudaError_t apply_sweep(ts_ctx* c, int kind, int scale_pow)
+cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow)
 {
     cudaError_t e = cudaSuccess;
     DiagOp d; d.present = (scale_pow != 0); d.alpha = TS_Z; d.t = 0.0; d.scale_pow = scale_pow;
@@ -679,7 +680,7 @@ cudaError_t apply_sweep(ts_ctx* c, int kind, int scale_pow)
     return e;
 }
 
-} // namespace
+extern "C" {
 
 int ts_energy(ts_ctx* c, double* out)
 {
@@ -689,12 +690,12 @@ int ts_energy(ts_ctx* c, double* out)
     // |(X^dag psi)_k|^2 (eq. 7, 10: P:81-84), the unnormalised sweeps carrying a factor 2^N in |.|^2.
     double ez = 0.0, ex = 0.0, ey = 0.0;
     cudaError_t e = ts_reduce_energy_diag(c, TS_Z, &ez);
-    if (e == cudaSuccess) e = apply_sweep(c, SW_YDAG, 0);
+    if (e == cudaSuccess) e = ts_apply_sweep_all(c, SW_YDAG, 0);
     if (e == cudaSuccess) e = ts_reduce_energy_diag(c, TS_X, &ex);
-    if (e == cudaSuccess) e = apply_sweep(c, SW_Y, -c->N);           // back: Y Y^dag = 2^N, removed exactly
-    if (e == cudaSuccess) e = apply_sweep(c, SW_XDAG, 0);
+    if (e == cudaSuccess) e = ts_apply_sweep_all(c, SW_Y, -c->N);           // back: Y Y^dag = 2^N, removed exactly
+    if (e == cudaSuccess) e = ts_apply_sweep_all(c, SW_XDAG, 0);
     if (e == cudaSuccess) e = ts_reduce_energy_diag(c, TS_Y, &ey);
-    if (e == cudaSuccess) e = apply_sweep(c, SW_X, -c->N);
+    if (e == cudaSuccess) e = ts_apply_sweep_all(c, SW_X, -c->N);
     if (e != cudaSuccess) return cuda_status(e);
     const double sc = ldexp(1.0, -c->N);
     *out = ez + sc * (ex + ey);

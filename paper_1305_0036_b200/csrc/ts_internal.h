@@ -64,6 +64,8 @@ struct ts_ctx {
     cudaStream_t stream;
     double h[3][TS_MAX_N];
     double Jeff[3][TS_MAX_N][TS_MAX_N];   // symmetric, zero diagonal: Jeff[j][k] = J[j][k] + J[k][j]  (A1)
+    double e0[3];     // energy offset added to E_alpha(k) by every diagonal: 0 for ts_create; for a shard context
+                      // (ts_shard_create) the fields and couplings of the spins that sit on the rank bits
     double* d_h;      // [3][TS_MAX_N]
     double* d_Jeff;   // [3][TS_MAX_N][TS_MAX_N]
     double2* psi;     // 2^N amplitudes (device)
@@ -110,6 +112,10 @@ struct ts_ctx {
 // (1 for a tile pass, 3 for a triple launch, N-bit fractions for the rest are not counted: 0).
 void ts_prof_begin(ts_ctx* c, int kc, double state_passes = 0.0);
 void ts_prof_end(ts_ctx* c);
+
+// One global rotation (sweep) of the whole local state, optionally followed by the exact scaling 2^scale_pow: every group
+// of the plan once (tiled), or one launch per spin (ts_api.cu).
+cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow);
 
 // ---- naive path (ts_naive.cu)
 cudaError_t ts_naive_rotate(ts_ctx* c, int j, int kind);

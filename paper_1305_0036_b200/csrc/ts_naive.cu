@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) k_naive_rotate(double2* __restrict__ psi,
 // (eq. 1 P:33 with A1/A2; eq. 9; on-the-fly evaluation).
 __global__ void __launch_bounds__(256) k_naive_diag(double2* __restrict__ psi, int N, uint64_t dim,
                                                     const double* __restrict__ h, const double* __restrict__ Jeff,
-                                                    double t, double scale)
+                                                    double t, double scale, double e0)
 {
     __shared__ double sh[TS_MAX_N];
     __shared__ double sJ[TS_MAX_N * TS_MAX_N];
@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(256) k_naive_diag(double2* __restrict__ psi, i
             E += sj * (sh[j] + f);     // each unordered pair once (m < j) with Jeff = J_jm + J_mj
         }
         double sn, cs;
-        sincos(-t * E, &sn, &cs);
+        sincos(-t * (E + e0), &sn, &cs);
         cs *= scale; sn *= scale;
         const double2 c = psi[k];
         psi[k] = make_double2(c.x * cs - c.y * sn, c.x * sn + c.y * cs);
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) k_naive_diag(double2* __restrict__ psi, i
 
 // E[k] = E_alpha(k) for all k (the stored vectors of P:119)
 __global__ void __launch_bounds__(256) k_build_energy(double* __restrict__ E, int N, uint64_t dim, const double* __restrict__ h,
-                                                      const double* __restrict__ Jeff)
+                                                      const double* __restrict__ Jeff, double e0)
 {
     __shared__ double sh[TS_MAX_N];
     __shared__ double sJ[TS_MAX_N * TS_MAX_N];
@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(256) k_build_energy(double* __restrict__ E, in
             for (int m = 0; m < j; ++m) f += sJ[j * N + m] * ((double)((k >> m) & 1) - 0.5);
             e += sj * (sh[j] + f);
         }
-        E[k] = e;
+        E[k] = e + e0;
     }
 }
 
@@ -152,7 +152,7 @@ cudaError_t ts_naive_diag(ts_ctx* c, const DiagOp& d)
             if (e != cudaSuccess) return e;
             ts_prof_begin(c, TS_KC_SETUP);
             k_build_energy<<<grid, 256, 0, c->stream>>>(c->d_energy[d.alpha], c->N, dim, c->d_h + d.alpha * TS_MAX_N,
-                                                        c->d_Jeff + (size_t)d.alpha * TS_MAX_N * TS_MAX_N);
+                                                        c->d_Jeff + (size_t)d.alpha * TS_MAX_N * TS_MAX_N, c->e0[d.alpha]);
             ts_prof_end(c);
         }
         ts_prof_begin(c, TS_KC_NAIVE_DIAG);
@@ -163,7 +163,7 @@ cudaError_t ts_naive_diag(ts_ctx* c, const DiagOp& d)
     ts_prof_begin(c, TS_KC_NAIVE_DIAG);
     k_naive_diag<<<grid, 256, 0, c->stream>>>(c->psi, c->N, dim, c->d_h + d.alpha * TS_MAX_N,
                                                c->d_Jeff + (size_t)d.alpha * TS_MAX_N * TS_MAX_N, d.t,
-                                               ldexp(1.0, d.scale_pow));
+                                               ldexp(1.0, d.scale_pow), c->e0[d.alpha]);
     ts_prof_end(c);
     return cudaGetLastError();
 }

@@ -22,6 +22,7 @@ struct SmallParams {
     int N, order;
     long long n_steps;
     double tau;
+    double e0[3];            // energy offsets of the context (zero unless it is a shard)
 };
 
 __device__ __forceinline__ void small_pair(int kind, double2& c0, double2& c1)
@@ -56,7 +57,7 @@ __global__ void __launch_bounds__(ST, 1) k_small_evolve(const SmallParams p)
                 for (int m = 0; m < j; ++m) f += J[j * TS_MAX_N + m] * ((double)((k >> m) & 1) - 0.5);
                 e += sj * f;
             }
-            E[a * dim + k] = e;
+            E[a * dim + k] = e + p.e0[a];
         }
         s[k] = p.psi[k];
     }
@@ -122,6 +123,7 @@ cudaError_t ts_small_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
     SmallParams p;
     p.psi = c->psi; p.h = c->d_h; p.Jeff = c->d_Jeff;
     p.N = c->N; p.order = order; p.n_steps = (long long)n_steps; p.tau = tau;
+    for (int a = 0; a < 3; ++a) p.e0[a] = c->e0[a];
     const size_t smem = (sizeof(double2) + 3 * sizeof(double)) << c->N;
     ts_prof_begin(c, TS_KC_SMALL);
     k_small_evolve<<<1, ST, smem, c->stream>>>(p);

@@ -24,7 +24,7 @@ cudaError_t g_init_status = cudaSuccess;
 // Geometry of the diagonal-time layout of one group: which spins sit on register bits (R), thread bits (T) and
 // outside the tile (X).
 struct PhaseGeom {
-    double t;
+    double t, e0;        // time of the diagonal; energy offset of the context (shards: the spins on the rank bits)
     int N, nfixed;
     int nr, nt;          // register bits / thread bits at diagonal time (5 + 7)
     int rec;             // entries of a tile-phase record (32)
@@ -42,7 +42,7 @@ inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : 1
 PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
 {
     PhaseGeom q;
-    q.t = t; q.N = c->N; q.nfixed = c->N - TS_TILE_LOG2;
+    q.t = t; q.e0 = 0.0; q.N = c->N; q.nfixed = c->N - TS_TILE_LOG2;
     q.nr = 5; q.nt = TS_TILE_LOG2 - q.nr; q.rec = 32;
     for (int b = 0; b < 5; ++b) q.rspin[b] = 0;
     for (int b = 0; b < 8; ++b) q.tspin[b] = 0;
@@ -128,6 +128,7 @@ __global__ void __launch_bounds__(256) k_build_tile_phase(double2* __restrict__ 
         double ar = 0.0;
         for (int i = 0; i < q.nr; ++i) ar += a_of(q.rspin[i]);
         E -= 0.5 * ar;
+        E += q.e0;
     } else if (e < 17) {
         const int v = e - 1;
         for (int b = 0; b < 4; ++b) E = fma((double)((v >> b) & 1) - 0.5, a_of(q.tspin[b]), E);
@@ -345,7 +346,8 @@ cudaError_t ts_tile_get_tables(ts_ctx* c, const DiagOp& d, int group, int layout
         ts_tile_free_tables(c);
     }
     const TileGroup& g = c->groups[group];
-    const PhaseGeom q = make_geom(c, g, d.t, layout);
+    PhaseGeom q = make_geom(c, g, d.t, layout);
+    q.e0 = c->e0[d.alpha];
     const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
     const int GT = 1 << q.nt, nrr = 1 << q.nr;
     const size_t n_thread_tab = (size_t)(1 + q.nr) * GT;          // TT, WT[nr]; RR[2^nr] follows

@@ -1,0 +1,223 @@
+"""One state vector sharded over G = 2^g GPUs (SURVEY 8 e, 8 f NEXT-5): binding of the ts_shard_* calls plus the collective.
+
+The method's arithmetic (rotations, diagonals, their sequence, the effective Hamiltonian of a shard) is the library's
+(csrc/ts_shard.cu).  This module supplies what joins the ranks:
+
+  * `alltoall_exchange`: the once-per-sweep index-bit swap as `torch.distributed.all_to_all_single` (NCCL over NVLink /
+    NVSwitch on GPUs; gloo in the CPU test): block rho' of a rank's shard goes to rank rho', block rho' of the result comes
+    from rank rho';
+  * `ShardedTrotterSuzuki`: one rank's shard (two device buffers, the ts_shard object, the exchange callback);
+  * `LocalCluster`: all G shards of a small system on ONE GPU, one Python thread per rank, the exchange done by plain
+    device copies between the shards -- how the sharded path is checked against the oracle on a single-GPU box;
+  * index bookkeeping to scatter / gather a full state and to assemble <S^z_j> over ranks.
+"""
+from __future__ import annotations
+
+import ctypes
+import threading
+from typing import Callable, List, Optional
+
+import numpy as np
+
+from . import binding as B
+
+
+def log2_exact(world: int) -> int:
+    g = int(world).bit_length() - 1
+    if world < 1 or (1 << g) != world:
+        raise ValueError(f"the number of ranks must be a power of two, got {world}")
+    return g
+
+
+def shard_slice(N: int, world: int, rank: int) -> slice:
+    """Layout 0: rank rho holds the amplitudes whose top g index bits equal rho, i.e. a contiguous slice."""
+    n = N - log2_exact(world)
+    return slice(rank << n, (rank + 1) << n)
+
+
+def alltoall_exchange(src, dst, group=None) -> None:
+    """Index-bit swap of the g rank bits with the top g local bits: equal-split all-to-all of the shard."""
+    import torch
+    import torch.distributed as dist
+    if src.is_complex():
+        src, dst = torch.view_as_real(src), torch.view_as_real(dst)
+    dist.all_to_all_single(dst, src, group=group)
+
+
+def assemble_sz(local_sz: np.ndarray, local_norm2: float, spin_of_bit: np.ndarray, n_local: int, rank: int) -> np.ndarray:
+    """This rank's contribution to <S^z_j> of every spin j of the full system: local bits carry what ts_expect_all(z)
+    summed over the shard; a spin on rank bit r has the fixed value bit_r(rank) - 1/2 on all of the shard's amplitudes."""
+    N = spin_of_bit.size
+    out = np.zeros(N)
+    for b in range(n_local):
+        out[spin_of_bit[b]] = local_sz[b]
+    for r in range(N - n_local):
+        out[spin_of_bit[n_local + r]] = (((rank >> r) & 1) - 0.5) * local_norm2
+    return out
+
+
+class ShardedTrotterSuzuki:
+    """Rank `rank` of `world` = 2^g: 2^(N-g) amplitudes on `device`.  `exchange(src, dst)` defaults to the NCCL all-to-all."""
+
+    def __init__(self, N: int, h, J, rank: int, world: int, device: str = "cuda:0",
+                 exchange: Optional[Callable] = None, group=None):
+        import torch
+        self._torch = torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the Trotter-Suzuki path has no CPU fallback")
+        self.N, self.rank, self.world, self.g = int(N), int(rank), int(world), log2_exact(world)
+        self.n = self.N - self.g
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self._lib = B.load()
+        h = np.ascontiguousarray(h, dtype=np.float64)
+        J = np.ascontiguousarray(J, dtype=np.float64)
+        if h.shape != (3, N) or J.shape != (3, N, N):
+            raise ValueError(f"h must be [3][{N}] and J [3][{N}][{N}]")
+        self._s = ctypes.c_void_p()
+        B._check(self._lib.ts_shard_create(ctypes.byref(self._s), N, h.ctypes.data_as(B._dp), J.ctypes.data_as(B._dp),
+                                           self.g, self.rank), "ts_shard_create")
+        self.buf = [torch.zeros(1 << self.n, dtype=torch.complex128, device=self.device) for _ in range(2)]
+        B._check(self._lib.ts_shard_bind(self._s, B._vp(self.buf[0].data_ptr()), B._vp(self.buf[1].data_ptr())), "ts_shard_bind")
+        B._check(self._lib.ts_shard_set_stream(self._s, B._vp(torch.cuda.current_stream(self.device).cuda_stream)),
+                 "ts_shard_set_stream")
+        self._exchange = exchange if exchange is not None else (lambda s, d: alltoall_exchange(s, d, group))
+        self._error = None
+        self._cb = B.EXCHANGE_FN(self._callback)       # keep the thunk alive as long as the shard
+
+    def _callback(self, user, src, dst) -> int:
+        try:
+            k = 0 if src == self.buf[0].data_ptr() else 1
+            self._exchange(self.buf[k], self.buf[k ^ 1])
+            return 0
+        except BaseException as exc:                   # never let an exception cross the C frame
+            self._error = exc
+            return 1
+
+    # ------------------------------------------------------------------ state
+    def info(self):
+        n, c, b = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        B._check(self._lib.ts_shard_info(self._s, ctypes.byref(n), ctypes.byref(c), ctypes.byref(b)), "ts_shard_info")
+        return n.value, c.value, b.value
+
+    def spin_map(self, config: int) -> np.ndarray:
+        out = (ctypes.c_int * self.N)()
+        B._check(self._lib.ts_shard_spin_map(self._s, config, out), "ts_shard_spin_map")
+        return np.array(list(out), dtype=np.int64)
+
+    def set_local_state(self, amps) -> None:
+        """`amps`: this rank's 2^(N-g) amplitudes in layout 0 (`full_state[shard_slice(N, world, rank)]`)."""
+        torch = self._torch
+        t = torch.as_tensor(np.ascontiguousarray(amps, dtype=np.complex128)) if not torch.is_tensor(amps) else amps
+        B._check(self._lib.ts_shard_bind(self._s, B._vp(self.buf[0].data_ptr()), B._vp(self.buf[1].data_ptr())), "ts_shard_bind")
+        self.buf[0].copy_(t.reshape(-1), non_blocking=False)
+
+    def local_state(self) -> np.ndarray:
+        _, cfg, b = self.info()
+        if cfg != 0:
+            raise RuntimeError("the shard is in layout 1 (mid-step); whole steps end in layout 0")
+        self._torch.cuda.synchronize(self.device)
+        return self.buf[b].cpu().numpy()
+
+    # ------------------------------------------------------------------ the hot path
+    def evolve(self, tau: float, n_steps: int, order: int = 4) -> None:
+        self._torch.cuda.set_device(self.device)       # (the current device is per thread)
+        self._error = None
+        st = self._lib.ts_shard_evolve(self._s, float(tau), int(n_steps), int(order), self._cb, None)
+        if self._error is not None:
+            raise self._error
+        B._check(st, "ts_shard_evolve")
+
+    # ------------------------------------------------------------------ observables (this rank's part; sums are all-reduces)
+    def local_sz_contribution(self) -> np.ndarray:
+        n, cfg, _ = self.info()
+        ctx = B._vp(self._lib.ts_shard_ctx(self._s, cfg))
+        sz = np.zeros(n)
+        B._check(self._lib.ts_expect_all(ctx, B.Z, sz.ctypes.data_as(B._dp)), "ts_expect_all")
+        nrm = ctypes.c_double()
+        B._check(self._lib.ts_norm2(ctx, ctypes.byref(nrm)), "ts_norm2")
+        return assemble_sz(sz, nrm.value, self.spin_map(cfg), n, self.rank)
+
+    def local_norm2(self) -> float:
+        _, cfg, _ = self.info()
+        nrm = ctypes.c_double()
+        B._check(self._lib.ts_norm2(B._vp(self._lib.ts_shard_ctx(self._s, cfg)), ctypes.byref(nrm)), "ts_norm2")
+        return nrm.value
+
+    def expect_z_all(self, group=None) -> np.ndarray:
+        """<S^z_j> of all N spins of the full system (an all-reduce over the ranks of `group`)."""
+        import torch.distributed as dist
+        t = self._torch.as_tensor(self.local_sz_contribution(), device=self.device)
+        dist.all_reduce(t, group=group)
+        return t.cpu().numpy()
+
+    def close(self) -> None:
+        if self._s:
+            self._lib.ts_shard_destroy(self._s)
+            self._s = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class LocalCluster:
+    """All 2^g shards of a small system on one GPU, one thread per rank; the exchange is done by device copies between
+    the shards (all on the same stream, so stream order is the only synchronisation the data needs; the thread barrier
+    makes sure every rank has issued its part of the sweep before anybody copies)."""
+
+    def __init__(self, N: int, h, J, world: int, device: str = "cuda:0"):
+        import torch
+        self._torch = torch
+        self.N, self.world = int(N), int(world)
+        self.device = torch.device(device)
+        self._barrier = threading.Barrier(world)
+        self._src: List = [None] * world
+        self.shards = [ShardedTrotterSuzuki(N, h, J, r, world, device, exchange=self._make_exchange(r)) for r in range(world)]
+
+    def _make_exchange(self, r: int):
+        def exchange(src, dst):
+            self._src[r] = src
+            self._barrier.wait(timeout=120)
+            blk = src.numel() // self.world
+            for rp in range(self.world):
+                dst[rp * blk:(rp + 1) * blk].copy_(self._src[rp][r * blk:(r + 1) * blk])
+            self._barrier.wait(timeout=120)
+        return exchange
+
+    def set_state(self, full: np.ndarray) -> None:
+        for r, s in enumerate(self.shards):
+            s.set_local_state(full[shard_slice(self.N, self.world, r)])
+
+    def get_state(self) -> np.ndarray:
+        return np.concatenate([s.local_state() for s in self.shards])
+
+    def evolve(self, tau: float, n_steps: int, order: int = 4) -> None:
+        errors: List = []
+
+        def run(s):
+            try:
+                s.evolve(tau, n_steps, order)
+            except BaseException as exc:
+                errors.append(exc)
+                self._barrier.abort()
+        threads = [threading.Thread(target=run, args=(s,)) for s in self.shards]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        self._torch.cuda.synchronize(self.device)
+        if errors:
+            raise errors[0]
+
+    def expect_z_all(self) -> np.ndarray:
+        return np.sum([s.local_sz_contribution() for s in self.shards], axis=0)
+
+    def norm2(self) -> float:
+        return float(sum(s.local_norm2() for s in self.shards))
+
+    def close(self) -> None:
+        for s in self.shards:
+            s.close()
