@@ -153,6 +153,9 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  *   TS_OPT_KERNEL          1 (default): warp-specialised TMA kernels; 0: one CTA per tile, register loads
  *   TS_OPT_CHUNK           1 (default): [high . fused low . high] as one L2-blocked launch where the plan allows; 0: off
  *   TS_OPT_CHUNK_MAX_LOG2  largest chunk of the L2-blocked launch, log2 amplitudes (default 21 = 32 MiB), 13..26
+ *   TS_OPT_CHUNK_MIN_LOG2  smallest chunk the L2-blocked launch is used for (default 21: only a full 9-bit group above A; with
+ *                          smaller chunks the per-chunk hand-overs between CTAs cost more than the HBM round trips they
+ *                          save, profiles/r02_tuner.md); the tests lower it to 13 to exercise those hand-overs
  *   TS_OPT_L2_PROMOTION    tensor-map L2 promotion of the high groups: 0 none (default), 1: 128 B, 2: 256 B
  *   TS_OPT_SMALL           1 (default): under TS_PLAN_AUTO, N <= 12 runs a whole ts_evolve call as one single-CTA launch
  *                          (state in shared memory; small systems are latency-bound); 0: tiled / naive plans
@@ -172,12 +175,13 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  *                          their shared-memory layout exchanges (wrong results by construction; time attribution only)
  * Errors: TS_ERR_ARG (unknown key, value out of range). */
 enum { TS_OPT_KERNEL = 0, TS_OPT_CHUNK = 1, TS_OPT_CHUNK_MAX_LOG2 = 2, TS_OPT_L2_PROMOTION = 3, TS_OPT_SMALL = 4,
-       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7, TS_OPT_PAIR = 8, TS_OPT_PROBE = 9 };
+       TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7, TS_OPT_PAIR = 8, TS_OPT_PROBE = 9,
+       TS_OPT_CHUNK_MIN_LOG2 = 10 };
 int ts_set_option(ts_ctx* ctx, int key, int value);
 int ts_get_option(ts_ctx* ctx, int key, int* value);
 
 /* Apply the line for this context's N of a plan file written by the tuner ("stored in a file"):
- *     N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 l2_promotion=0
+ *     N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 chunk_min_log2=21 l2_promotion=0
  * (text; '#' starts a comment line; keys other than N may be omitted).  No line for this N: TS_OK, nothing changes.
  * ts_create applies the file named by the environment variable TS_PLAN_FILE, if set, the same way.
  * Errors: TS_ERR_ARG (file cannot be opened, or the line does not describe a valid plan for N). */

@@ -203,6 +203,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->opt_kernel = env_int("TS_KERNEL", 1);
     c->opt_chunk = env_int("TS_CHUNK3", 1);
     c->opt_chunk_max_log2 = env_int("TS_CHUNK3_MAX_LOG2", 21);
+    c->opt_chunk_min_log2 = env_int("TS_CHUNK3_MIN_LOG2", 21);
     c->opt_small = env_int("TS_SMALL", 1);
     c->opt_diag_source = 0;
     c->opt_l2_promotion = env_int("TS_L2_PROMOTION", 0);
@@ -363,6 +364,7 @@ int ts_set_option(ts_ctx* c, int key, int value)
     case TS_OPT_MAX_CTAS: if (value < 0) return TS_ERR_ARG; c->opt_max_ctas = value; break;
     case TS_OPT_L2_HINTS: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_l2_hints = value; break;
     case TS_OPT_PAIR: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_pair = value; break;
+    case TS_OPT_CHUNK_MIN_LOG2: if (value < TS_TILE_LOG2 + 1 || value > 26) return TS_ERR_ARG; c->opt_chunk_min_log2 = value; break;
     case TS_OPT_PROBE: if (value < 0 || value > 3) return TS_ERR_ARG; c->opt_probe = value; break;
     case TS_OPT_DIAG_SOURCE:
         if (value < 0 || value > 1) return TS_ERR_ARG;
@@ -395,6 +397,7 @@ int ts_get_option(ts_ctx* c, int key, int* value)
     case TS_OPT_MAX_CTAS: *value = c->opt_max_ctas; break;
     case TS_OPT_L2_HINTS: *value = c->opt_l2_hints; break;
     case TS_OPT_PAIR: *value = c->opt_pair; break;
+    case TS_OPT_CHUNK_MIN_LOG2: *value = c->opt_chunk_min_log2; break;
     case TS_OPT_PROBE: *value = c->opt_probe; break;
     default: return TS_ERR_ARG;
     }
@@ -402,7 +405,7 @@ int ts_get_option(ts_ctx* c, int key, int* value)
 }
 
 // Plan file (the tuned sequence of rotations per N "stored in a file"): text, one line per system size,
-//     N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 l2_promotion=0
+//     N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 chunk_min_log2=21 l2_promotion=0
 // `groups` = bits of every high group, bottom to top (ts_set_plan_groups); the other keys are ts_set_option values and
 // may be omitted.  Lines starting with '#' are comments.  Returns TS_OK and leaves the context untouched when the file
 // has no line for this N.
@@ -417,7 +420,7 @@ int ts_load_plan_file(ts_ctx* c, const char* path)
         if (line[0] == '#') continue;
         int n = -1;
         std::vector<int> groups;
-        int kernel = -1, chunk = -1, cmax = -1, prom = -1;
+        int kernel = -1, chunk = -1, cmax = -1, cmin = -1, prom = -1;
         bool have_groups = false;
         for (char* tok = strtok(line, " \t\r\n"); tok; tok = strtok(nullptr, " \t\r\n")) {
             if (!strncmp(tok, "N=", 2)) n = atoi(tok + 2);
@@ -432,12 +435,14 @@ int ts_load_plan_file(ts_ctx* c, const char* path)
             else if (!strncmp(tok, "kernel=", 7)) kernel = atoi(tok + 7);
             else if (!strncmp(tok, "chunk=", 6)) chunk = atoi(tok + 6);
             else if (!strncmp(tok, "chunk_max_log2=", 15)) cmax = atoi(tok + 15);
+            else if (!strncmp(tok, "chunk_min_log2=", 15)) cmin = atoi(tok + 15);
             else if (!strncmp(tok, "l2_promotion=", 13)) prom = atoi(tok + 13);
         }
         if (n != c->N) continue;
         if (kernel >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_KERNEL, kernel);
         if (chunk >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_CHUNK, chunk);
         if (cmax >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_CHUNK_MAX_LOG2, cmax);
+        if (cmin >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_CHUNK_MIN_LOG2, cmin);
         if (prom >= 0 && st == TS_OK) st = ts_set_option(c, TS_OPT_L2_PROMOTION, prom);
         if (have_groups && st == TS_OK && c->N >= TS_TILE_LOG2 + 1) st = ts_set_plan_groups(c, (int)groups.size(), groups.data());
         break;

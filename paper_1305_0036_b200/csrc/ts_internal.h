@@ -79,6 +79,7 @@ struct ts_ctx {
     int opt_kernel;                      // 1: v2 pipelined kernels where the geometry allows, 0: k_tile_pass only
     int opt_chunk;                       // 1: L2-blocked triple launches
     int opt_chunk_max_log2;              // largest chunk (log2 amplitudes)
+    int opt_chunk_min_log2;              // smallest chunk the triple launch is used for (profiles/r02_tuner.md)
     int opt_small;                       // 1: single-CTA path for N <= 12
     int opt_diag_source;                 // 0: factorised on-the-fly tables, 1: stored 2^N phase vectors, naive plan only
     int opt_l2_promotion;                // tensor-map L2 promotion of the high groups: 0 none, 1 128 B, 2 256 B

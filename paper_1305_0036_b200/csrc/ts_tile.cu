@@ -438,6 +438,7 @@ bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
     if (g.g0 != TS_TILE_LOG2 || !v2_geometry_ok(g)) return false;     // the group right above A
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
     if (C >= c->N || C > c->opt_chunk_max_log2) return false;          // at least two chunks, each small enough for L2
+    if (C < c->opt_chunk_min_log2) return false;                       // small chunks: the hand-overs cost more than the round trips
     const int v = (ka == SW_YDAG && kb == SW_Y) ? 0 : (ka == SW_X && kb == SW_XDAG) ? 1 : -1;
     return v >= 0 && g_v2_chunk[g.s == 3 ? 1 : 0][v] != nullptr;
 }

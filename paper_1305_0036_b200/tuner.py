@@ -63,8 +63,9 @@ def candidates(N: int, max_groups: int = 4, max_splits: int = 12) -> List[dict]:
 
 
 def plan_line(N: int, plan: dict) -> str:
+    cmin = 12 + plan["groups"][0] if (plan["chunk"] and plan["groups"]) else 21      # the chunk this plan was timed with
     return (f"N={N} groups={','.join(str(b) for b in plan['groups'])} kernel={plan['kernel']} chunk={plan['chunk']} "
-            f"chunk_max_log2=21 l2_promotion={plan['l2_promotion']}")
+            f"chunk_max_log2=21 chunk_min_log2={min(cmin, 21)} l2_promotion={plan['l2_promotion']}")
 
 
 def time_plan(ts, B, plan: dict, tau: float, steps: int, repeats: int) -> float:
@@ -72,6 +73,7 @@ def time_plan(ts, B, plan: dict, tau: float, steps: int, repeats: int) -> float:
     import torch
     ts.set_option(B.OPT_KERNEL, plan["kernel"])
     ts.set_option(B.OPT_CHUNK, plan["chunk"])
+    ts.set_option(B.OPT_CHUNK_MIN_LOG2, 13)       # a candidate with chunk = 1 is timed WITH the triple launch, whatever its chunk size
     ts.set_option(B.OPT_L2_PROMOTION, plan["l2_promotion"])
     ts.set_plan_groups(plan["groups"])
     ts.evolve(tau, 1, 4)                      # builds the phase tables, warms up

@@ -74,6 +74,7 @@ def test_triple_launch_generic_J_full_oracle(B, N, groups, order, family):
     w = W.generic(N, seed=500 + 7 * N + len(groups) + order, tau=0.02, n_steps=steps, order=order, symmetric_fill=(N % 3 == 0))
     ts = B.TrotterSuzuki(N, w.h, w.J)
     ts.set_option(B.OPT_KERNEL, family)
+    ts.set_option(B.OPT_CHUNK_MIN_LOG2, 13)        # small chunks on purpose: many hand-overs between CTAs per launch
     ts.set_plan_groups(groups)
     ts.set_state(w.state())
     ts.reset_profile()
@@ -116,6 +117,7 @@ def test_kernel_families_agree_and_match_oracle(B, N, groups):
         ts.set_plan_groups(groups)
         ts.set_option(B.OPT_KERNEL, kernel)
         ts.set_option(B.OPT_CHUNK, chunk)
+        ts.set_option(B.OPT_CHUNK_MIN_LOG2, 13)
         assert ts.get_option(B.OPT_KERNEL) == kernel
         ts.set_state(w.state())
         ts.reset_profile()
@@ -139,6 +141,7 @@ def test_few_ctas_walk_many_tiles(B, N, groups, max_ctas, family):
     ts.set_plan_groups(groups)
     ts.set_option(B.OPT_KERNEL, family)
     ts.set_option(B.OPT_MAX_CTAS, max_ctas)
+    ts.set_option(B.OPT_CHUNK_MIN_LOG2, 13)
     ts.set_state(w.state())
     ts.evolve(w.tau, 2, 4)
     check_amps(ts.get_state(), oracle_run(w, 2, 4))
@@ -152,6 +155,7 @@ def test_triple_launch_repeated_in_one_process(B):
         w = W.generic(N, seed=7000 + rep, tau=0.02, n_steps=4)
         ts = B.TrotterSuzuki(N, w.h, w.J)
         ts.set_option(B.OPT_MAX_CTAS, (0, 37, 100)[rep % 3])
+        ts.set_option(B.OPT_CHUNK_MIN_LOG2, 13)
         ts.set_plan_groups([2, 4] if rep % 2 else [3, 3])
         ts.set_state(w.state())
         ts.reset_profile()

@@ -30,7 +30,8 @@ def test_candidates_put_the_default_plan_first_and_stay_bounded():
 
 def test_plan_line_format():
     line = T.plan_line(30, {"groups": [9, 9], "chunk": 1, "l2_promotion": 2, "kernel": 1})
-    assert line == "N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 l2_promotion=2"
+    assert line == "N=30 groups=9,9 kernel=1 chunk=1 chunk_max_log2=21 chunk_min_log2=21 l2_promotion=2"
+    assert "chunk_min_log2=16" in T.plan_line(20, {"groups": [4, 2, 2], "chunk": 1, "l2_promotion": 0, "kernel": 1})
 
 
 @pytest.mark.gpu
