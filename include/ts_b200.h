@@ -150,12 +150,18 @@ int ts_set_plan(ts_ctx* ctx, int mode, int run_bits, int max_group_bits);
 int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
 
 /* Execution options (all have defaults; the tuner and the A/B benchmarks set them).
- *   TS_OPT_KERNEL          1 (default): warp-specialised TMA kernels; 0: one CTA per tile, register loads
+ *   TS_OPT_KERNEL          2 (default): automatic -- the warp-specialised persistent TMA kernels when every SM
+ *                          walks more than two tiles (N >= 21 on a B200), else one CTA per tile with register loads (the
+ *                          pipeline's set-up does not pay for one or two tiles); 1: TMA kernels always; 0: never
  *   TS_OPT_CHUNK           1 (default): [high . fused low . high] as one L2-blocked launch where the plan allows; 0: off
  *   TS_OPT_CHUNK_MAX_LOG2  largest chunk of the L2-blocked launch, log2 amplitudes (default 21 = 32 MiB), 13..26
  *   TS_OPT_CHUNK_MIN_LOG2  smallest chunk the L2-blocked launch is used for (default 21: only a full 9-bit group above A; with
  *                          smaller chunks the per-chunk hand-overs between CTAs cost more than the HBM round trips they
  *                          save, profiles/r02_tuner.md); the tests lower it to 13 to exercise those hand-overs
+ *   TS_OPT_GRAPH           1 (default): for N <= TS_OPT_GRAPH_MAX_N (default 21: L2-resident, launch-bound states) a
+ *                          ts_evolve call of >= 4 steps captures the launches of one step into a CUDA graph and replays it;
+ *                          0: every launch goes to the stream one by one.  Off while profiling is on.
+ *   TS_OPT_GRAPH_MAX_N     see above (12..33).   TS_OPT_GRAPH_REPLAYS (read-only): graph replays so far
  *   TS_OPT_L2_PROMOTION    tensor-map L2 promotion of the high groups: 0 none (default), 1: 128 B, 2: 256 B
  *   TS_OPT_SMALL           1 (default): under TS_PLAN_AUTO, N <= 12 runs a whole ts_evolve call as one single-CTA launch
  *                          (state in shared memory; small systems are latency-bound); 0: tiled / naive plans
@@ -176,7 +182,7 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  * Errors: TS_ERR_ARG (unknown key, value out of range). */
 enum { TS_OPT_KERNEL = 0, TS_OPT_CHUNK = 1, TS_OPT_CHUNK_MAX_LOG2 = 2, TS_OPT_L2_PROMOTION = 3, TS_OPT_SMALL = 4,
        TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7, TS_OPT_PAIR = 8, TS_OPT_PROBE = 9,
-       TS_OPT_CHUNK_MIN_LOG2 = 10 };
+       TS_OPT_CHUNK_MIN_LOG2 = 10, TS_OPT_GRAPH = 11, TS_OPT_GRAPH_MAX_N = 12, TS_OPT_GRAPH_REPLAYS = 13 };
 int ts_set_option(ts_ctx* ctx, int key, int value);
 int ts_get_option(ts_ctx* ctx, int key, int* value);
 

@@ -135,6 +135,197 @@ int ensure_state(ts_ctx* c)
     return TS_OK;
 }
 
+// The executable graph of the last graph-mode call is destroyed once its replays have completed.
+void graph_release(ts_ctx* c)
+{
+    if (!c->g_exec) return;
+    if (c->g_done) cudaEventSynchronize(c->g_done);
+    cudaGraphExecDestroy(c->g_exec);
+    c->g_exec = nullptr;
+}
+
+// ---- the tiled path's launch stream -------------------------------------------------------------------------------
+// Passes are generated sweep by sweep (the paper's runs are 5e5 .. 5e6 steps: no list of them is ever
+// materialised for a long run) and emitted through a three-entry window in which the pattern
+//     [H1 single ka] [A fused ka . D . kb] [H1 single kb]   ->   one L2-blocked launch (ts_tile_v2.cuh)
+// is recognised.  A command is one launch: a tile pass or a triple launch.
+struct Cmd {
+    int triple;        // 1: ts_tile_chunk_triple(gi, k1, d, k2), 0: ts_tile_pass(gi, k1, d or none, k2)
+    int gi, k1, k2;
+    DiagOp d;
+    bool operator==(const Cmd& o) const
+    {
+        return triple == o.triple && gi == o.gi && k1 == o.k1 && k2 == o.k2 && d.present == o.d.present &&
+               (!d.present || (d.alpha == o.d.alpha && d.t == o.d.t && d.scale_pow == o.d.scale_pow));
+    }
+};
+
+template <class Emit>
+cudaError_t generate(ts_ctx* c, const Seq& q, Emit&& emit)
+{
+    struct Pass { int gi, k1, k2; DiagOp d; };
+    const int g = (int)c->groups.size();
+    int64_t sweep = 1;                 // next sweep to expand
+    int pos = 0;                       // next position within it
+    Pass win[4];
+    int nwin = 0;
+    cudaError_t e = cudaSuccess;
+    auto refill = [&]() {
+        while (nwin < 3 && sweep <= q.M) {
+            const int64_t i = sweep;
+            Pass ps; ps.d.present = 0; ps.gi = 0; ps.k1 = SW_NONE; ps.k2 = SW_NONE;
+            bool out = true;
+            if (g == 1) {
+                if (pos == 0) { ps.d = q.diag(i - 1); ps.k2 = q.kind(i); }
+                else { ps.d = q.diag(q.M); }                                // trailing diagonal after the last sweep
+                ++pos;
+                if (pos > (i == q.M ? 1 : 0)) { ++sweep; pos = 0; }
+            } else {
+                const bool fwd = (i & 1);
+                const bool first = (pos == 0), last = (pos == g - 1);
+                ps.gi = fwd ? pos : g - 1 - pos;
+                if (first && i > 1) out = false;                               // done by the previous fused pass
+                else if (last && i < q.M) { ps.k1 = q.kind(i); ps.d = q.diag(i); ps.k2 = q.kind(i + 1); }
+                else if (first && i == 1) { ps.d = q.diag(0); ps.k2 = q.kind(1); }
+                else if (last && i == q.M) { ps.k1 = q.kind(i); ps.d = q.diag(q.M); }
+                else ps.k1 = q.kind(i);
+                if (++pos == g) { ++sweep; pos = 0; }
+            }
+            if (out) win[nwin++] = ps;
+        }
+    };
+    for (;;) {
+        refill();
+        if (nwin == 0 || e != cudaSuccess) break;
+        int used = 1;
+        Cmd cmd;
+        if (nwin >= 3) {
+            const Pass &p0 = win[0], &p1 = win[1], &p2 = win[2];
+            if (p0.gi == p2.gi && p1.gi == 0 && p0.k2 == SW_NONE && !p0.d.present && p2.k2 == SW_NONE && !p2.d.present &&
+                p1.d.present && p1.k1 == p0.k1 && p1.k2 == p2.k1 && ts_tile_chunk_supported(c, p0.gi, p1.k1, p1.k2)) {
+                cmd.triple = 1; cmd.gi = p0.gi; cmd.k1 = p1.k1; cmd.k2 = p1.k2; cmd.d = p1.d;
+                used = 3;
+            }
+        }
+        if (used == 1) { cmd.triple = 0; cmd.gi = win[0].gi; cmd.k1 = win[0].k1; cmd.k2 = win[0].k2; cmd.d = win[0].d; }
+        e = emit(cmd);
+        for (int k = used; k < nwin; ++k) win[k - used] = win[k];
+        nwin -= used;
+    }
+    return e;
+}
+
+cudaError_t execute(ts_ctx* c, const Cmd& cmd)
+{
+    if (cmd.triple) return ts_tile_chunk_triple(c, cmd.gi, cmd.k1, cmd.d, cmd.k2);
+    return ts_tile_pass(c, cmd.gi, cmd.k1, cmd.d.present ? &cmd.d : nullptr, cmd.k2);
+}
+
+bool coop_refused(cudaError_t e)
+{
+    return e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources || e == cudaErrorNotSupported;
+}
+
+// Small, L2-resident states are launch-bound (a tile pass at N = 16 lasts ~5 us, the gap between two
+// dependent launches about as long).  The launch stream of a run is periodic, head + unit x (n - 2) + tail with `unit` =
+// one 4th-order step, so the unit is captured ONCE into a CUDA graph and replayed.  The decomposition is found by
+// generating the streams of 2, 3 and 4 steps on the host and is checked on the 4-step stream before it is trusted.
+bool split_periodic(ts_ctx* c, const Seq& q, std::vector<Cmd>& head, std::vector<Cmd>& unit, std::vector<Cmd>& tail)
+{
+    std::vector<Cmd> L[3];
+    for (int k = 0; k < 3; ++k) {
+        const Seq qk(q.order, q.N, q.tau, 2 + k);
+        if (generate(c, qk, [&](const Cmd& cmd) { L[k].push_back(cmd); return cudaSuccess; }) != cudaSuccess) return false;
+    }
+    if (L[1].size() <= L[0].size() || L[2].size() - L[1].size() != L[1].size() - L[0].size()) return false;
+    const size_t P = L[1].size() - L[0].size();
+    size_t S = 0;                                       // common suffix of the 2- and 3-step streams
+    while (S < L[0].size() && L[0][L[0].size() - 1 - S] == L[1][L[1].size() - 1 - S]) ++S;
+    if (S == 0 || S >= L[0].size()) return false;
+    const size_t H = L[0].size() - S;
+    head.assign(L[0].begin(), L[0].begin() + H);
+    tail.assign(L[0].begin() + H, L[0].end());
+    unit.assign(L[1].begin() + H, L[1].begin() + H + P);
+    std::vector<Cmd> check(head);                       // head + unit + unit + tail must be the 4-step stream
+    check.insert(check.end(), unit.begin(), unit.end());
+    check.insert(check.end(), unit.begin(), unit.end());
+    check.insert(check.end(), tail.begin(), tail.end());
+    if (check.size() != L[2].size()) return false;
+    for (size_t k = 0; k < check.size(); ++k) if (!(check[k] == L[2][k])) return false;
+    return true;
+}
+
+int evolve_tiled(ts_ctx* c, const Seq& q)
+{
+    cudaError_t e = cudaSuccess;
+    auto run = [&](const Cmd& cmd) -> cudaError_t {
+        cudaError_t r = execute(c, cmd);
+        if (cmd.triple && coop_refused(r)) {
+            // not all CTAs can be co-resident here (MPS, a shared GPU): run the three passes one by one from now on
+            cudaGetLastError();
+            c->opt_chunk = 0;
+            r = ts_tile_pass(c, cmd.gi, cmd.k1, nullptr, SW_NONE);
+            if (r == cudaSuccess) r = ts_tile_pass(c, 0, cmd.k1, &cmd.d, cmd.k2);
+            if (r == cudaSuccess) r = ts_tile_pass(c, cmd.gi, cmd.k2, nullptr, SW_NONE);
+        }
+        return r;
+    };
+    const int64_t n_steps = q.n_sub / (q.order == 4 ? 5 : 1);
+    const bool graph_ok = c->opt_graph && !c->profiling && c->N <= c->opt_graph_max_n && n_steps >= 4;
+    std::vector<Cmd> head, unit, tail;
+    if (graph_ok && split_periodic(c, q, head, unit, tail)) {
+        for (const Cmd& cmd : head) { e = run(cmd); if (e != cudaSuccess) return cuda_status(e); }
+        // every phase table of the unit exists before the capture starts (building one allocates and launches)
+        c->dry_run = 1;
+        for (const Cmd& cmd : unit) { e = execute(c, cmd); if (e != cudaSuccess) break; }
+        c->dry_run = 0;
+        if (e != cudaSuccess) return cuda_status(e);
+        graph_release(c);
+        int64_t l0[TS_KC_COUNT]; double t0[TS_KC_COUNT];
+        memcpy(l0, c->launches, sizeof(l0)); memcpy(t0, c->tiles_acc, sizeof(t0));
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t gexec = nullptr;
+        bool captured = false;
+        // capture on a stream of our own (the caller's may be the legacy default stream, which cannot be captured); nothing
+        // runs there: the graph is launched into the caller's stream
+        cudaStream_t user = c->stream;
+        if (!c->g_stream && cudaStreamCreateWithFlags(&c->g_stream, cudaStreamNonBlocking) != cudaSuccess) c->g_stream = nullptr;
+        if (c->g_stream && cudaStreamBeginCapture(c->g_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            c->stream = c->g_stream;
+            cudaError_t ce = cudaSuccess;
+            for (const Cmd& cmd : unit) { ce = execute(c, cmd); if (ce != cudaSuccess) break; }
+            cudaError_t ee = cudaStreamEndCapture(c->g_stream, &graph);
+            c->stream = user;
+            if (ce == cudaSuccess && ee == cudaSuccess && graph && cudaGraphInstantiate(&gexec, graph, 0) == cudaSuccess)
+                captured = true;
+        }
+        cudaGetLastError();
+        if (graph) cudaGraphDestroy(graph);
+        int64_t left = n_steps - 2;
+        if (captured) {
+            // the capture went through the launchers once: count its launches once per replay
+            for (int k = 0; k < TS_KC_COUNT; ++k) {
+                c->launches[k] = l0[k] + (c->launches[k] - l0[k]) * left;
+                c->tiles_acc[k] = t0[k] + (c->tiles_acc[k] - t0[k]) * (double)left;
+            }
+            c->graph_replays += left;
+            for (; left > 0 && e == cudaSuccess; --left) e = cudaGraphLaunch(gexec, c->stream);
+            c->g_exec = gexec;
+            if (!c->g_done) cudaEventCreateWithFlags(&c->g_done, cudaEventDisableTiming);
+            if (c->g_done) cudaEventRecord(c->g_done, c->stream);
+        } else {
+            memcpy(c->launches, l0, sizeof(l0)); memcpy(c->tiles_acc, t0, sizeof(t0));
+            if (gexec) cudaGraphExecDestroy(gexec);
+        }
+        for (; left > 0 && e == cudaSuccess; --left)  // capture refused: the same launches, one by one
+            for (const Cmd& cmd : unit) { e = run(cmd); if (e != cudaSuccess) break; }
+        for (const Cmd& cmd : tail) { if (e != cudaSuccess) break; e = run(cmd); }
+        return cuda_status(e);
+    }
+    e = generate(c, q, run);
+    return cuda_status(e);
+}
+
 } // namespace
 
 void ts_prof_begin(ts_ctx* c, int kc, double state_passes)
@@ -200,7 +391,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->plan_mode = TS_PLAN_AUTO; c->run_bits = 0; c->max_group_bits = 0;
     // execution options: defaults, overridable once per context from the environment (A/B runs of bench.py) and at
     // any time through ts_set_option
-    c->opt_kernel = env_int("TS_KERNEL", 1);
+    c->opt_kernel = env_int("TS_KERNEL", 2);
     c->opt_chunk = env_int("TS_CHUNK3", 1);
     c->opt_chunk_max_log2 = env_int("TS_CHUNK3_MAX_LOG2", 21);
     c->opt_chunk_min_log2 = env_int("TS_CHUNK3_MIN_LOG2", 21);
@@ -210,6 +401,11 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->opt_max_ctas = 0;
     c->opt_l2_hints = env_int("TS_L2_HINTS", 1);
     c->opt_pair = env_int("TS_PAIR", 1);
+    c->opt_graph = env_int("TS_GRAPH", 1);
+    c->opt_graph_max_n = 21;
+    c->dry_run = 0;
+    c->g_exec = nullptr; c->g_done = nullptr; c->g_stream = nullptr;
+    c->graph_replays = 0;
     c->opt_probe = 0;
     c->d_chunk_ctr = nullptr; c->chunk_ctr_cap = 0;
     c->d_sched = nullptr;
@@ -247,6 +443,9 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
 int ts_destroy(ts_ctx* c)
 {
     if (!c) return TS_OK;
+    graph_release(c);
+    if (c->g_done) cudaEventDestroy(c->g_done);
+    if (c->g_stream) cudaStreamDestroy(c->g_stream);
     if (c->psi && c->owns_psi) cudaFree(c->psi);
     if (c->d_h) cudaFree(c->d_h);
     if (c->d_Jeff) cudaFree(c->d_Jeff);
@@ -357,13 +556,15 @@ int ts_set_option(ts_ctx* c, int key, int value)
 {
     if (!c) return TS_ERR_ARG;
     switch (key) {
-    case TS_OPT_KERNEL: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_kernel = value; break;
+    case TS_OPT_KERNEL: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_kernel = value; break;
     case TS_OPT_CHUNK: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_chunk = value; break;
     case TS_OPT_CHUNK_MAX_LOG2: if (value < TS_TILE_LOG2 + 1 || value > 26) return TS_ERR_ARG; c->opt_chunk_max_log2 = value; break;
     case TS_OPT_L2_PROMOTION: if (value < 0 || value > 2) return TS_ERR_ARG; c->opt_l2_promotion = value; c->tmaps.clear(); break;
     case TS_OPT_MAX_CTAS: if (value < 0) return TS_ERR_ARG; c->opt_max_ctas = value; break;
     case TS_OPT_L2_HINTS: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_l2_hints = value; break;
     case TS_OPT_PAIR: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_pair = value; break;
+    case TS_OPT_GRAPH: if (value < 0 || value > 1) return TS_ERR_ARG; c->opt_graph = value; break;
+    case TS_OPT_GRAPH_MAX_N: if (value < TS_TILE_LOG2 || value > TS_MAX_N) return TS_ERR_ARG; c->opt_graph_max_n = value; break;
     case TS_OPT_CHUNK_MIN_LOG2: if (value < TS_TILE_LOG2 + 1 || value > 26) return TS_ERR_ARG; c->opt_chunk_min_log2 = value; break;
     case TS_OPT_PROBE: if (value < 0 || value > 3) return TS_ERR_ARG; c->opt_probe = value; break;
     case TS_OPT_DIAG_SOURCE:
@@ -397,6 +598,9 @@ int ts_get_option(ts_ctx* c, int key, int* value)
     case TS_OPT_MAX_CTAS: *value = c->opt_max_ctas; break;
     case TS_OPT_L2_HINTS: *value = c->opt_l2_hints; break;
     case TS_OPT_PAIR: *value = c->opt_pair; break;
+    case TS_OPT_GRAPH: *value = c->opt_graph; break;
+    case TS_OPT_GRAPH_MAX_N: *value = c->opt_graph_max_n; break;
+    case TS_OPT_GRAPH_REPLAYS: *value = (int)(c->graph_replays > 0x7fffffff ? 0x7fffffff : c->graph_replays); break;
     case TS_OPT_CHUNK_MIN_LOG2: *value = c->opt_chunk_min_log2; break;
     case TS_OPT_PROBE: *value = c->opt_probe; break;
     default: return TS_ERR_ARG;
@@ -472,7 +676,7 @@ int ts_describe_plan(ts_ctx* c, char* buf, int buflen)
             else snprintf(tmp, sizeof tmp, " H[spins %d..%d, run 2^%d]", t.g0, t.g0 + TS_TILE_LOG2 - t.s - 1, t.s);
             s += tmp;
         }
-        snprintf(tmp, sizeof tmp, "; kernels=%s", c->opt_kernel ? "v2" : "v1");
+        snprintf(tmp, sizeof tmp, "; kernels=%s", ts_tile_layout_for(c, 0, SW_YDAG, SW_Y) ? "v2" : "v1");
         s += tmp;
         if (ts_tile_chunk_supported(c, 1, SW_YDAG, SW_Y)) {
             const TileGroup& t = c->groups[1];
@@ -502,63 +706,7 @@ int ts_evolve(ts_ctx* c, double tau, int64_t n_steps, int order)
         return cuda_status(e);
     }
 
-    // ---- passes are generated sweep by sweep (the paper's runs are 5e5 .. 5e6 steps: no list of them
-    // is ever materialised) and executed through a three-entry window in which the pattern
-    //     [H1 single ka] [A fused ka . D . kb] [H1 single kb]   ->   one L2-blocked launch (ts_tile_v2.cuh)
-    // is recognised.
-    struct Pass { int gi, k1, k2; DiagOp d; };
-    const int g = (int)c->groups.size();
-    int64_t sweep = 1;                 // next sweep to expand
-    int pos = 0;                       // next position within it
-    Pass win[4];
-    int nwin = 0;
-    auto refill = [&]() {
-        while (nwin < 3 && sweep <= q.M) {
-            const int64_t i = sweep;
-            Pass ps; ps.d.present = 0; ps.gi = 0; ps.k1 = SW_NONE; ps.k2 = SW_NONE;
-            bool emit = true;
-            if (g == 1) {
-                if (pos == 0) { ps.d = q.diag(i - 1); ps.k2 = q.kind(i); }
-                else { ps.d = q.diag(q.M); }                                // trailing diagonal after the last sweep
-                ++pos;
-                if (pos > (i == q.M ? 1 : 0)) { ++sweep; pos = 0; }
-            } else {
-                const bool fwd = (i & 1);
-                const bool first = (pos == 0), last = (pos == g - 1);
-                ps.gi = fwd ? pos : g - 1 - pos;
-                if (first && i > 1) emit = false;                              // done by the previous fused pass
-                else if (last && i < q.M) { ps.k1 = q.kind(i); ps.d = q.diag(i); ps.k2 = q.kind(i + 1); }
-                else if (first && i == 1) { ps.d = q.diag(0); ps.k2 = q.kind(1); }
-                else if (last && i == q.M) { ps.k1 = q.kind(i); ps.d = q.diag(q.M); }
-                else ps.k1 = q.kind(i);
-                if (++pos == g) { ++sweep; pos = 0; }
-            }
-            if (emit) win[nwin++] = ps;
-        }
-    };
-    for (;;) {
-        refill();
-        if (nwin == 0 || e != cudaSuccess) break;
-        int used = 1;
-        if (nwin >= 3) {
-            const Pass &p0 = win[0], &p1 = win[1], &p2 = win[2];
-            if (p0.gi == p2.gi && p1.gi == 0 && p0.k2 == SW_NONE && !p0.d.present && p2.k2 == SW_NONE && !p2.d.present &&
-                p1.d.present && p1.k1 == p0.k1 && p1.k2 == p2.k1 && ts_tile_chunk_supported(c, p0.gi, p1.k1, p1.k2)) {
-                e = ts_tile_chunk_triple(c, p0.gi, p1.k1, p1.d, p1.k2);
-                if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources || e == cudaErrorNotSupported) {
-                    cudaGetLastError();          // not all CTAs can be co-resident here (MPS, a shared GPU): run the
-                    c->opt_chunk = 0;            // three passes one by one from now on
-                    e = cudaSuccess;
-                } else {
-                    used = 3;
-                }
-            }
-        }
-        if (used == 1) e = ts_tile_pass(c, win[0].gi, win[0].k1, win[0].d.present ? &win[0].d : nullptr, win[0].k2);
-        for (int k = used; k < nwin; ++k) win[k - used] = win[k];
-        nwin -= used;
-    }
-    return cuda_status(e);
+    return evolve_tiled(c, q);
 }
 
 int ts_evolve_observe(ts_ctx* c, double tau, int64_t n_steps, int order, int alpha, int j, double* out)

@@ -76,7 +76,7 @@ struct ts_ctx {
     std::vector<TileGroup> groups;
     int use_small;                       // N <= 12 under TS_PLAN_AUTO: the single-CTA path (ts_small.cu)
     // execution options (ts_set_option)
-    int opt_kernel;                      // 1: v2 pipelined kernels where the geometry allows, 0: k_tile_pass only
+    int opt_kernel;                      // 0: k_tile_pass only, 1: v2 pipelined kernels where the geometry allows, 2: v2 from three tiles per SM on
     int opt_chunk;                       // 1: L2-blocked triple launches
     int opt_chunk_max_log2;              // largest chunk (log2 amplitudes)
     int opt_chunk_min_log2;              // smallest chunk the triple launch is used for (profiles/r02_tuner.md)
@@ -85,6 +85,13 @@ struct ts_ctx {
     int opt_l2_promotion;                // tensor-map L2 promotion of the high groups: 0 none, 1 128 B, 2 256 B
     int opt_max_ctas;                    // upper bound on the persistent kernels' grid (0: one CTA per SM)
     int opt_l2_hints;                    // L2 eviction priorities on the TMA transfers of the L2-blocked launch
+    int opt_graph;                       // 1: small states replay one step's launches from a CUDA graph (ts_api.cu)
+    int opt_graph_max_n;                 // largest N that does so
+    int dry_run;                         // launchers build / look up their phase tables and return without launching
+    cudaGraphExec_t g_exec;              // the graph of the last graph-mode ts_evolve call (released lazily, after g_done)
+    cudaEvent_t g_done;
+    cudaStream_t g_stream;               // capture-only stream
+    int64_t graph_replays;               // graph launches so far (each = one 4th-order step's launches)
     int opt_pair;                        // tickets of a high group are pairs of adjacent tiles
     int opt_probe;                       // copy-only tile passes (the compute groups skip the tile body): pipeline ceilings
     unsigned int* d_sched;               // [2] ticket counter + finished-CTA counter of the persistent kernels (zero between launches)

@@ -382,6 +382,9 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
 {
     const TileGroup& g = c->groups[group];
     if (c->opt_kernel == 0 || !v2_geometry_ok(g)) return 0;
+    // automatic choice: the persistent pipeline pays once every SM walks several tiles; with at most two tiles per SM
+    // (N <= 20 on 148 SMs) the one-CTA-per-tile kernel is faster (no pipeline set-up: 283 vs 361 us per step at N = 20)
+    if (c->opt_kernel == 2 && (((uint64_t)1 << (c->N - TS_TILE_LOG2)) <= 2ull * (uint64_t)c->num_sms)) return 0;
     return g_v2[v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
@@ -414,6 +417,7 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
         if (e != cudaSuccess) return e;
         const uint64_t cap = (c->opt_max_ctas > 0 && c->opt_max_ctas < c->num_sms) ? (uint64_t)c->opt_max_ctas : (uint64_t)c->num_sms;
         const uint64_t grid = ntiles < cap ? ntiles : cap;
+        if (c->dry_run) return cudaSuccess;
         ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
         kern<<<(unsigned)grid, TS_V2_THREADS, TS_V2_SMEM, c->stream>>>(p, tm);
         ts_prof_end(c);
@@ -424,6 +428,7 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
     tile_kernel_t k = g_tab[kind1][kind2];
     if (!k) return cudaErrorInvalidValue;
     const size_t smem = p.two_stage ? (sizeof(double2) << TS_TILE_LOG2) : 0;
+    if (c->dry_run) return cudaSuccess;
     ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
     k<<<(unsigned)ntiles, TS_TILE_THREADS, smem, c->stream>>>(p);
     ts_prof_end(c);
@@ -434,6 +439,7 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
 bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
 {
     if (c->opt_chunk == 0 || c->opt_kernel == 0 || gh != 1 || (int)c->groups.size() < 3 || !c->groups[0].is_low) return false;
+    if (ts_tile_layout_for(c, 0, ka, kb) == 0) return false;           // the TMA kernels are not in use at this size
     const TileGroup& g = c->groups[gh];
     if (g.g0 != TS_TILE_LOG2 || !v2_geometry_ok(g)) return false;     // the group right above A
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
@@ -454,6 +460,7 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
         e = ts_tile_get_tables(c, d, 0, 1, &tb);
         if (e != cudaSuccess) return e;
     }
+    if (c->dry_run) return cudaSuccess;
     const size_t nctr = 2 * (size_t)nchunks;
     if (c->chunk_ctr_cap < nctr) {
         e = cudaStreamSynchronize(c->stream);                          // queued launches may still use the old counters

@@ -26,8 +26,10 @@ def B():
     return binding
 
 
-def run_gpu(B, w, n_steps=None, order=None, plan=None, tau=None):
+def run_gpu(B, w, n_steps=None, order=None, plan=None, tau=None, kernel=None):
     ts = B.TrotterSuzuki(w.N, w.h, w.J)
+    if kernel is not None:
+        ts.set_option(B.OPT_KERNEL, kernel)
     if plan is not None:
         ts.set_plan(*plan)
     ts.set_state(w.state())
@@ -100,10 +102,14 @@ TILED_CASES = [
 ]
 
 
+# kernel 1: the TMA kernels at every size; 2: the library's own choice (one CTA per tile up to two tiles per SM)
+@pytest.mark.parametrize("kernel", [1, 2])
 @pytest.mark.parametrize("N,rb,mg", TILED_CASES)
-def test_tiled_generic(B, N, rb, mg):
+def test_tiled_generic(B, N, rb, mg, kernel):
     w = W.generic(N, seed=200 + N, tau=0.02, n_steps=2 if N < 20 else 1, order=4, symmetric_fill=(N == 16))
-    ts = run_gpu(B, w, plan=(B.PLAN_TILED, rb, mg))
+    ts = run_gpu(B, w, plan=(B.PLAN_TILED, rb, mg), kernel=kernel)
+    if N >= 13:
+        assert ("kernels=v2" in ts.describe_plan()) == (kernel == 1 or N >= 21)
     ref = run_oracle(w)
     check_amps(ts.get_state(), ref)
     if N <= 18:
@@ -113,7 +119,7 @@ def test_tiled_generic(B, N, rb, mg):
 @pytest.mark.parametrize("N", [12, 14, 18])
 def test_tiled_order2_and_negative_tau(B, N):
     w = W.generic(N, seed=300 + N, tau=0.03, n_steps=3, order=2)
-    ts = run_gpu(B, w)
+    ts = run_gpu(B, w, kernel=1)
     ref = run_oracle(w)
     check_amps(ts.get_state(), ref)
     # echo: evolving back with -tau returns the initial state (U_2, U_4 are palindromic)

@@ -154,6 +154,7 @@ def test_triple_launch_repeated_in_one_process(B):
     for rep in range(30):
         w = W.generic(N, seed=7000 + rep, tau=0.02, n_steps=4)
         ts = B.TrotterSuzuki(N, w.h, w.J)
+        ts.set_option(B.OPT_KERNEL, 1)
         ts.set_option(B.OPT_MAX_CTAS, (0, 37, 100)[rep % 3])
         ts.set_option(B.OPT_CHUNK_MIN_LOG2, 13)
         ts.set_plan_groups([2, 4] if rep % 2 else [3, 3])
@@ -386,3 +387,30 @@ def test_naive_plan_with_stored_energy_vectors(B, N):
         assert ts.get_profile()["naive_rot"]["launches"] == 2 * 20 * N
         ts.close()
     assert np.max(np.abs(out[0] - out[1])) <= 1e-13
+
+
+# --------------------------------------------------------------------------------------------- CUDA-graph replay (small states)
+@pytest.mark.parametrize("N,kernel", [(13, 2), (16, 2), (16, 1), (19, 2), (21, 2)])
+@pytest.mark.parametrize("order", [4, 2])
+def test_graph_replay_of_small_states(B, N, kernel, order):
+    """N <= 21: a call of >= 4 steps replays one step's launches from a CUDA graph (head + unit x (n - 2) + tail).  Same
+    amplitudes, bit for bit, as the launch-by-launch path, and both against the oracle; the launch counters count the
+    replayed launches."""
+    steps = 6
+    w = W.generic(N, seed=9000 + N + order, tau=0.02, n_steps=steps, order=order)
+    out = []
+    for graph in (1, 0):
+        ts = B.TrotterSuzuki(N, w.h, w.J)
+        ts.set_option(B.OPT_KERNEL, kernel)
+        ts.set_option(B.OPT_GRAPH, graph)
+        ts.set_state(w.state())
+        ts.reset_profile()
+        ts.evolve(w.tau, steps, order)
+        prof = ts.get_profile()
+        assert ts.get_option(B.OPT_GRAPH_REPLAYS) == (steps - 2 if graph else 0)
+        out.append((ts.get_state(), sum(v["launches"] for v in prof.values())))
+        ts.evolve(w.tau, 1, order)                 # a later call on the same context (the graph is released lazily)
+        ts.close()
+    assert out[0][1] == out[1][1]                  # same number of kernel launches accounted
+    assert np.array_equal(out[0][0], out[1][0])
+    check_amps(out[0][0], oracle_run(w, steps, order))
