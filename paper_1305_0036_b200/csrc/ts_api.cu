@@ -407,6 +407,8 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->g_exec = nullptr; c->g_done = nullptr; c->g_stream = nullptr;
     c->graph_replays = 0;
     c->opt_probe = 0;
+    c->opt_groups = env_int("TS_GROUPS", 2);
+    if (c->opt_groups < 1 || c->opt_groups > 2) c->opt_groups = 2;
     c->d_chunk_ctr = nullptr; c->chunk_ctr_cap = 0;
     c->d_sched = nullptr;
     c->d_energy[0] = c->d_energy[1] = c->d_energy[2] = nullptr;

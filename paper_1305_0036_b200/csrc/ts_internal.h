@@ -93,6 +93,7 @@ struct ts_ctx {
     cudaStream_t g_stream;               // capture-only stream
     int64_t graph_replays;               // graph launches so far (each = one 4th-order step's launches)
     int opt_pair;                        // tickets of a high group are pairs of adjacent tiles
+    int opt_groups;                      // compute groups per CTA of the persistent kernels (2; 1 = experiment)
     int opt_probe;                       // copy-only tile passes (the compute groups skip the tile body): pipeline ceilings
     unsigned int* d_sched;               // [2] ticket counter + finished-CTA counter of the persistent kernels (zero between launches)
     unsigned int* d_chunk_ctr;           // done counters of the triple launch

@@ -407,6 +407,7 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
         p.sched = c->d_sched;
         p.pair_log2 = (c->opt_pair && !g.is_low && g.g0 > g.s && ntiles >= 2) ? 1u : 0u;   // adjacent tiles exist (nmid >= 1)
         p.probe = (c->opt_probe == 1);
+        p.ngroups = c->opt_groups;
         v2_kernel_t kern = g_v2[v2_type(g)][kind1][kind2];
         if (c->opt_probe >= 2) {                       // measurement builds exist for the fused passes of the N = 30 plan
             if (v2_type(g) == 2 && fused) kern = g_probe_H[c->opt_probe - 2];     // (the kinds do not change the cost)
@@ -478,6 +479,7 @@ cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int
     q.done = c->d_chunk_ctr;
     q.sched = c->d_sched;
     q.probe = (c->opt_probe == 1);
+    q.ngroups = c->opt_groups;
     q.nchunks = nchunks; q.tiles_log2 = (uint32_t)(C - TS_TILE_LOG2);
     q.l2_hints = c->opt_l2_hints;
     e = cudaMemsetAsync(c->d_chunk_ctr, 0, sizeof(unsigned int) * nctr, c->stream);

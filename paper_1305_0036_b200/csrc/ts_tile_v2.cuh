@@ -41,7 +41,9 @@
 #define TS_V2_THREADS 384                 // two compute warpgroups (8 warps) + one producer warpgroup (loader warp, storer warp, 2 idle)
 #define TS_V2_REGS_COMPUTE 232            // setmaxnreg: 256 x 232 + 128 x 40 = 64 512 <= 65 536 registers
 #define TS_V2_REGS_PRODUCER 40
+#ifndef TS_V2_NBUF
 #define TS_V2_NBUF 3
+#endif
 #define TS_V2_TILE_BYTES 65536
 #define TS_V2_OFF_TP (TS_V2_NBUF * TS_V2_TILE_BYTES)         // 3 x 512 B tile-phase records
 #define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3], tab mbarriers (80 B), then tile[3] (u32)
@@ -89,6 +91,7 @@ struct V2Pass {
     unsigned int* sched;         // [2]: next ticket, CTAs finished (both zero between launches: the last CTA resets them)
     uint32_t pair_log2;          // tiles per ticket = 2^pair_log2 (1: adjacent tile pairs of a high group)
     int probe;                   // 1: copy only -- the compute groups skip the tile body (TS_OPT_PROBE: pipeline ceilings)
+    int ngroups;                 // compute groups in use: 2, or 1 (TS_OPT_GROUPS: one tile at a time in arithmetic, two buffers in transport)
 };
 
 // L2-blocked triple launch: [high group, sweep KA] [group A: KA . D . KB] [high group, sweep KB] chunk by chunk.
@@ -99,6 +102,7 @@ struct V2Chunk {
     unsigned int* sched;         // [2]: next ticket, CTAs finished
     uint32_t nchunks, tiles_log2;
     int probe;
+    int ngroups;
     int l2_hints;                // 1: eviction priorities on the TMA transfers (keep a chunk in L2 until its third phase wrote it)
 };
 
@@ -616,7 +620,8 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
         const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
         const double scale = p.d.scale;
         if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
-        for (uint64_t j = grp;; j += 2) {
+        if (grp >= p.ngroups) return;
+        for (uint64_t j = grp;; j += p.ngroups) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
             v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
             const bool end = (v2_ld_tile(smraw, b) == TS_V2_END);
@@ -749,7 +754,8 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
         const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
         const double scale = q.d.scale;
         if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
-        for (uint64_t j = grp;; j += 2) {
+        if (grp >= q.ngroups) return;
+        for (uint64_t j = grp;; j += q.ngroups) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
             v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
             const uint32_t n = v2_ld_tile(smraw, b);
