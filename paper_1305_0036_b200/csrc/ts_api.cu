@@ -279,6 +279,7 @@ int evolve_tiled(ts_ctx* c, const Seq& q)
         c->dry_run = 1;
         for (const Cmd& cmd : unit) { e = execute(c, cmd); if (e != cudaSuccess) break; }
         c->dry_run = 0;
+    c->top_bits_only = 0;
         if (e != cudaSuccess) return cuda_status(e);
         graph_release(c);
         int64_t l0[TS_KC_COUNT]; double t0[TS_KC_COUNT];
@@ -404,6 +405,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->opt_graph = env_int("TS_GRAPH", 1);
     c->opt_graph_max_n = 21;
     c->dry_run = 0;
+    c->top_bits_only = 0;
     c->g_exec = nullptr; c->g_done = nullptr; c->g_stream = nullptr;
     c->graph_replays = 0;
     c->opt_probe = 0;

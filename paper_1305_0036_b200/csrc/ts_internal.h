@@ -87,6 +87,7 @@ struct ts_ctx {
     int opt_l2_hints;                    // L2 eviction priorities on the TMA transfers of the L2-blocked launch
     int opt_graph;                       // 1: small states replay one step's launches from a CUDA graph (ts_api.cu)
     int opt_graph_max_n;                 // largest N that does so
+    int top_bits_only;                   // > 0 (transient, ts_shard.cu): a high-group pass butterflies only its top so-many bits
     int dry_run;                         // launchers build / look up their phase tables and return without launching
     cudaGraphExec_t g_exec;              // the graph of the last graph-mode ts_evolve call (released lazily, after g_done)
     cudaEvent_t g_done;

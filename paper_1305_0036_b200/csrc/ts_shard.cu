@@ -22,8 +22,9 @@
 // The exchange itself is the caller's: a callback that moves 2^n amplitudes from `src` to `dst` (both device buffers on
 // this rank) through whatever joins the ranks -- NCCL all-to-all over NVLink in paper_1305_0036_b200/sharded.py, plain
 // copies between the shards of one GPU in the single-GPU test.  Everything else (sequence, rotations, diagonals) is this
-// library's own kernels.  This first version runs the sweeps unfused (one pass per bit group, one per diagonal); fusing
-// [top-spin rotation . D . next sweep's top group] and moving the exchange into the kernel over peer memory come next.
+// library's own kernels.  Per sweep a shard makes one tile pass per bit group plus ONE pass that rotates the arriving spins
+// and applies the diagonal (the top group's pass restricted to its top g bits); fusing that pass with the next sweep's
+// top group and moving the exchange into the kernel over peer memory come next.
 #include <math.h>
 #include <string.h>
 
@@ -92,6 +93,28 @@ cudaError_t rotate_range(ts_ctx* c, int kind, int first, int count)
     cudaError_t e = cudaSuccess;
     for (int j = first; j < first + count && e == cudaSuccess; ++j) e = ts_naive_rotate(c, j, kind);
     return e;
+}
+
+// The g spins that arrived with an exchange sit on the top g local bits, i.e. on the top bits of the plan's last bit
+// group: their rotation and the diagonal that follows the sweep are ONE tile pass of that group restricted to those bits.
+// (Shards below 12 spins, or a top group with fewer than g bits: one launch per spin, then the diagonal.)
+cudaError_t rotate_arrivals_then_diagonal(ts_ctx* c, int kind, int g, const DiagOp& d)
+{
+    if (!c->groups.empty() && c->groups.size() >= 2) {
+        const int last = (int)c->groups.size() - 1;
+        const TileGroup& tg = c->groups[last];
+        if (TS_TILE_LOG2 - tg.s >= g) {
+            c->top_bits_only = g;
+            cudaError_t e = ts_tile_pass(c, last, kind, d.present ? &d : nullptr, SW_NONE);
+            c->top_bits_only = 0;
+            return e;
+        }
+    }
+    cudaError_t e = cudaSuccess;
+    for (int j = c->N - g; j < c->N && e == cudaSuccess; ++j) e = ts_naive_rotate(c, j, kind);
+    if (e != cudaSuccess || !d.present) return e;
+    if (!c->groups.empty()) return ts_tile_pass(c, 0, SW_NONE, &d, SW_NONE);
+    return ts_naive_diag(c, d);
 }
 
 cudaError_t diagonal(ts_ctx* c, const DiagOp& d)
@@ -204,16 +227,6 @@ int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exch
         const int kind = kinds[(i - 1) & 3];
         e = rotate_range(s->cfg[s->cur_cfg], kind, 0, s->n);
         if (e != cudaSuccess) break;
-        if (s->g > 0) {
-            double2* src = s->buf[s->cur_buf];
-            double2* dst = s->buf[s->cur_buf ^ 1];
-            if (exchange(user, (void*)src, (void*)dst) != 0) return TS_ERR_CUDA;
-            s->cur_buf ^= 1; s->cur_cfg ^= 1;
-            ts_bind_state(s->cfg[0], (void*)dst);
-            ts_bind_state(s->cfg[1], (void*)dst);
-            e = rotate_range(s->cfg[s->cur_cfg], kind, s->n - s->g, s->g);
-            if (e != cudaSuccess) break;
-        }
         const int64_t u = (i - 1) >> 2;
         const double su = sub(u);
         switch ((i - 1) & 3) {
@@ -222,7 +235,17 @@ int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exch
         case 2: d.alpha = TS_Y; d.t = 0.5 * su; d.scale_pow = -s->N; break;
         default: d.alpha = TS_Z; d.t = 0.5 * su + 0.5 * sub(u + 1); d.scale_pow = -s->N; break;
         }
-        e = diagonal(s->cfg[s->cur_cfg], d);
+        if (s->g > 0) {
+            double2* src = s->buf[s->cur_buf];
+            double2* dst = s->buf[s->cur_buf ^ 1];
+            if (exchange(user, (void*)src, (void*)dst) != 0) return TS_ERR_CUDA;
+            s->cur_buf ^= 1; s->cur_cfg ^= 1;
+            ts_bind_state(s->cfg[0], (void*)dst);
+            ts_bind_state(s->cfg[1], (void*)dst);
+            e = rotate_arrivals_then_diagonal(s->cfg[s->cur_cfg], kind, s->g, d);
+        } else {
+            e = diagonal(s->cfg[s->cur_cfg], d);
+        }
     }
     return cuda_status(e);
 }

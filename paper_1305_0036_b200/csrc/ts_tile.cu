@@ -240,15 +240,17 @@ void fill_v1_params(const ts_ctx* c, const TileGroup& g, const DiagTables* tb, T
         for (int r = 0; r < 32; ++r) p->RR[r] = make_double2(1.0, 0.0);
     }
     p->s = g.s; p->g0 = g.g0;
-    const int nb = n_bfly(g);
+    // butterflied bits: all of the group's, or (c->top_bits_only > 0) only its top `top_bits_only` ones; the layouts the
+    // tile moves through -- and with them the diagonal's tables -- are those of the whole group either way
+    const int nb = (c->top_bits_only > 0 && !g.is_low) ? c->top_bits_only : n_bfly(g);
     p->two_stage = two_stage(g) ? 1 : 0;
     p->nshfl = g.is_low ? 2 : 0;
     if (g.is_low) { p->bf1 = 31u; p->bf2 = 31u; }
-    else if (nb <= 5) { p->bf1 = (31u << (5 - nb)) & 31u; p->bf2 = 0u; }          // top nb bits of f 7..11
+    else if (nb <= 5) { p->bf1 = (31u << (5 - nb)) & 31u; p->bf2 = 0u; }          // top nb bits of f 7..11 (layout 1)
     else { p->bf1 = 31u; p->bf2 = (31u << (10 - nb)) & 31u; }                       // top nb-5 bits of f 2..6
 }
 
-void fill_v2_geom(const TileGroup& g, V2Geom* q)
+void fill_v2_geom(const TileGroup& g, V2Geom* q, int top_bits_only = 0)
 {
     q->type = g.is_low ? 0 : 1;
     q->s = g.s; q->g0 = g.g0;
@@ -257,8 +259,9 @@ void fill_v2_geom(const TileGroup& g, V2Geom* q)
     q->two_stage = (!g.is_low && q->m > 5) ? 1 : 0;
     q->mask1 = 0u; q->mask2 = 0u;
     if (!g.is_low) {
-        q->mask1 = tsk::v2_h_mask1(q->m);
-        q->mask2 = tsk::v2_h_mask2(q->m);   // (H2 register bit 4 = f 7 is a filler)
+        const int mb = top_bits_only > 0 ? top_bits_only : q->m;          // f bits 12 - mb .. 11 are butterflied
+        q->mask1 = tsk::v2_h_mask1(mb);
+        q->mask2 = tsk::v2_h_mask2(mb);     // (H2 register bit 4 = f 7 is a filler)
     }
 }
 
@@ -385,7 +388,7 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
     // automatic choice: the persistent pipeline pays once every SM walks several tiles; with at most two tiles per SM
     // (N <= 20 on 148 SMs) the one-CTA-per-tile kernel is faster (no pipeline set-up: 283 vs 361 us per step at N = 20)
     if (c->opt_kernel == 2 && (((uint64_t)1 << (c->N - TS_TILE_LOG2)) <= 2ull * (uint64_t)c->num_sms)) return 0;
-    return g_v2[v2_type(g)][kind1][kind2] ? 1 : 0;
+    return g_v2[(c->top_bits_only > 0 && !g.is_low) ? 1 : v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
 cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int kind2)
@@ -401,14 +404,15 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
     const bool fused = (kind1 != SW_NONE && kind2 != SW_NONE);
     if (layout >= 1) {
         V2Pass p;
-        fill_v2_geom(g, &p.g);
+        const int tbo = g.is_low ? 0 : c->top_bits_only;
+        fill_v2_geom(g, &p.g, tbo);
         fill_v2_diag(tb, &p.d);
         p.ntiles = ntiles;
         p.sched = c->d_sched;
         p.pair_log2 = (c->opt_pair && !g.is_low && g.g0 > g.s && ntiles >= 2) ? 1u : 0u;   // adjacent tiles exist (nmid >= 1)
         p.probe = (c->opt_probe == 1);
         p.ngroups = c->opt_groups;
-        v2_kernel_t kern = g_v2[v2_type(g)][kind1][kind2];
+        v2_kernel_t kern = g_v2[tbo > 0 ? 1 : v2_type(g)][kind1][kind2];   // (a bit subset needs the run-time-mask kernels)
         if (c->opt_probe >= 2) {                       // measurement builds exist for the fused passes of the N = 30 plan
             if (v2_type(g) == 2 && fused) kern = g_probe_H[c->opt_probe - 2];     // (the kinds do not change the cost)
             if (v2_type(g) == 0 && fused) kern = g_probe_A[c->opt_probe - 2];

@@ -51,6 +51,13 @@ def test_sharded_matches_full_oracle(S, N, world, order):
     run_case(S, N, world, order, steps=2, seed=4000 + 10 * N + world)
 
 
+@pytest.mark.parametrize("N,world", [(22, 8), (21, 2)])
+def test_sharded_with_multi_group_shards(S, N, world):
+    """Shards of 19 / 20 spins: several bit groups per shard, a two-stage top group, and the arriving spins rotated by
+    the top group's tile pass restricted to its top g bits (fused with the diagonal)."""
+    run_case(S, N, world, 4, steps=1, seed=4700 + N)
+
+
 def test_one_rank_is_the_unsharded_path(S):
     run_case(S, 13, 1, 4, steps=1, seed=4500)
 
