@@ -96,8 +96,11 @@ int build_plan(ts_ctx* c)
             bits.push_back(mgmax);
             left -= mgmax;
         }
-        // ... and the bits above are split evenly: the longest runs for every remaining pass
-        const int ng = (left + mgmax - 1) / mgmax;
+        // ... and the bits above are split evenly: the longest runs for every remaining pass.  One bit too
+        // many for a single group (N = 31) is still ONE group, with 64-byte runs: measured 597 vs 673 ms per step against
+        // two groups of five (profiles/r02_ab_and_sizes.md) -- a tile pass more per sweep costs more than short runs do.
+        const bool ten = (c->run_bits == 0 && c->max_group_bits == 0 && left == mgmax + 1);
+        const int ng = ten ? 1 : (left + mgmax - 1) / mgmax;
         for (int i = 0; i < ng; ++i) bits.push_back(left / ng + (i < left % ng ? 1 : 0));
     }
     int g0 = TS_TILE_LOG2;

@@ -132,9 +132,24 @@ def test_cluster_factorisation_N30_bench_plan(B):
     assert "A[spins 0..11]" in plan and "3 group" in plan and "L2-blocked" in plan
 
 
+def test_cluster_factorisation_N31_default_plan(B):
+    """N = 31: the default plan puts ten bits (64-byte runs) into one top group instead of splitting them."""
+    import gc
+    import torch
+    gc.collect()
+    torch.cuda.empty_cache()                 # give back what earlier tests' tensors left in torch's caching allocator
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40 * 2 ** 30:
+        pytest.skip("needs 40 GiB of free device memory")
+    check_clustered(B, 31, 3, 1, seed=31, n_windows=32)
+
+
 def test_cluster_factorisation_N32_in_place(B):
     """64 GiB state, in place (config 5's size)."""
+    import gc
     import torch
+    gc.collect()
+    torch.cuda.empty_cache()                 # give back what earlier tests' tensors left in torch's caching allocator
     free, _ = torch.cuda.mem_get_info()
     if free < 80 * 2 ** 30:
         pytest.skip("needs 80 GiB of free device memory")
@@ -164,7 +179,10 @@ def test_config5_grid32_properties(B):
     """BASELINE config 5 Hamiltonian and checkerboard Neel state at N = 32: properties that hold at any size.
     Norm is conserved to 1e-12; the echo (U_4 is palindromic, so U_4(-tau) U_4(tau) = 1 exactly) returns the
     Neel state: c_Neel = 1 and <S^z_j> = -+1/2 again.  (Oracle parity at this size: the cluster test above.)"""
+    import gc
     import torch
+    gc.collect()
+    torch.cuda.empty_cache()                 # give back what earlier tests' tensors left in torch's caching allocator
     free, _ = torch.cuda.mem_get_info()
     if free < 80 * 2 ** 30:
         pytest.skip("needs 80 GiB of free device memory")
@@ -209,7 +227,10 @@ def test_N33_in_place_largest_state(B):
     """The largest state the ABI accepts (N = 33: 128 GiB, in place): the plan has four groups (A + 9 + 6 + 6), the state
     index needs 33 bits and byte offsets 37.  Properties that hold at any size, on the config-5 lattice recipe grown to
     3 x 11: norm conserved, the echo returns the Neel basis state exactly, <S^z_j> = -+1/2 again."""
+    import gc
     import torch
+    gc.collect()
+    torch.cuda.empty_cache()                 # give back what earlier tests' tensors left in torch's caching allocator
     free, _ = torch.cuda.mem_get_info()
     if free < 150 * 2 ** 30:
         pytest.skip("needs 150 GiB of free device memory")
