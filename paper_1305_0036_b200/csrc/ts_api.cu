@@ -409,7 +409,7 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     c->opt_graph_max_n = 21;
     c->dry_run = 0;
     c->top_bits_only = 0;
-    c->g_exec = nullptr; c->g_done = nullptr; c->g_stream = nullptr;
+    c->g_exec = nullptr; c->g_done = nullptr; c->g_stream = nullptr; c->d_row_ctr = nullptr;
     c->graph_replays = 0;
     c->opt_probe = 0;
     c->opt_groups = env_int("TS_GROUPS", 2);
@@ -453,6 +453,7 @@ int ts_destroy(ts_ctx* c)
     graph_release(c);
     if (c->g_done) cudaEventDestroy(c->g_done);
     if (c->g_stream) cudaStreamDestroy(c->g_stream);
+    if (c->d_row_ctr) cudaFree(c->d_row_ctr);
     if (c->psi && c->owns_psi) cudaFree(c->psi);
     if (c->d_h) cudaFree(c->d_h);
     if (c->d_Jeff) cudaFree(c->d_Jeff);
@@ -733,7 +734,54 @@ int ts_evolve_observe(ts_ctx* c, double tau, int64_t n_steps, int order, int alp
     }
     double* d_trace = c->d_trace;
     int st = TS_OK;
-    for (int64_t k = 0; k < n_steps && st == TS_OK; ++k) {
+    int64_t k = 0;
+    // Small states (launch-bound): the first step runs launch by launch (it builds every phase table and the
+    // reduction scratch), then [one step + the row's reduction] is captured once and replayed; the row index lives on
+    // the device and advances with every replay.
+    if (c->opt_graph && !c->profiling && c->N <= c->opt_graph_max_n && n_steps >= 4) {
+        st = ts_evolve(c, tau, 1, order);
+        if (st == TS_OK) st = cuda_status(ts_reduce_trace_row(c, alpha, j < 0 ? 0 : j, d_trace));
+        k = 1;
+        if (st == TS_OK && !c->d_row_ctr && cudaMalloc(&c->d_row_ctr, sizeof(unsigned int)) != cudaSuccess) { cudaGetLastError(); c->d_row_ctr = nullptr; }
+        if (st == TS_OK && c->d_row_ctr) {
+            graph_release(c);
+            cudaStream_t user = c->stream;
+            cudaGraph_t graph = nullptr;
+            cudaGraphExec_t gexec = nullptr;
+            int64_t l0[TS_KC_COUNT]; double t0[TS_KC_COUNT];
+            memcpy(l0, c->launches, sizeof(l0)); memcpy(t0, c->tiles_acc, sizeof(t0));
+            bool captured = false;
+            if (!c->g_stream && cudaStreamCreateWithFlags(&c->g_stream, cudaStreamNonBlocking) != cudaSuccess) c->g_stream = nullptr;
+            if (c->g_stream && cudaStreamBeginCapture(c->g_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                c->stream = c->g_stream;
+                int cs = ts_evolve(c, tau, 1, order);
+                if (cs == TS_OK) cs = cuda_status(ts_reduce_trace_row(c, alpha, j < 0 ? 0 : j, d_trace, c->d_row_ctr));
+                cudaError_t ee = cudaStreamEndCapture(c->g_stream, &graph);
+                c->stream = user;
+                if (cs == TS_OK && ee == cudaSuccess && graph && cudaGraphInstantiate(&gexec, graph, 0) == cudaSuccess) captured = true;
+            }
+            cudaGetLastError();
+            if (graph) cudaGraphDestroy(graph);
+            if (captured) {
+                const int64_t left = n_steps - 1;
+                for (int q = 0; q < TS_KC_COUNT; ++q) {
+                    c->launches[q] = l0[q] + (c->launches[q] - l0[q]) * left;
+                    c->tiles_acc[q] = t0[q] + (c->tiles_acc[q] - t0[q]) * (double)left;
+                }
+                cudaError_t e2 = ts_set_u32(c, c->d_row_ctr, 1u);
+                for (; k < n_steps && e2 == cudaSuccess; ++k) e2 = cudaGraphLaunch(gexec, c->stream);
+                c->graph_replays += left;
+                c->g_exec = gexec;
+                if (!c->g_done) cudaEventCreateWithFlags(&c->g_done, cudaEventDisableTiming);
+                if (c->g_done) cudaEventRecord(c->g_done, c->stream);
+                st = cuda_status(e2);
+            } else {
+                memcpy(c->launches, l0, sizeof(l0)); memcpy(c->tiles_acc, t0, sizeof(t0));
+                if (gexec) cudaGraphExecDestroy(gexec);
+            }
+        }
+    }
+    for (; k < n_steps && st == TS_OK; ++k) {
         st = ts_evolve(c, tau, 1, order);
         if (st == TS_OK) st = cuda_status(ts_reduce_trace_row(c, alpha, j < 0 ? 0 : j, d_trace + (size_t)k * TS_TRACE_STRIDE));
     }

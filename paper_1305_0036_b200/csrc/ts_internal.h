@@ -92,6 +92,7 @@ struct ts_ctx {
     cudaGraphExec_t g_exec;              // the graph of the last graph-mode ts_evolve call (released lazily, after g_done)
     cudaEvent_t g_done;
     cudaStream_t g_stream;               // capture-only stream
+    unsigned int* d_row_ctr;             // next trace row (ts_evolve_observe replayed from a graph)
     int64_t graph_replays;               // graph launches so far (each = one 4th-order step's launches)
     int opt_pair;                        // tickets of a high group are pairs of adjacent tiles
     int opt_groups;                      // compute groups per CTA of the persistent kernels (2; 1 = experiment)
@@ -159,4 +160,5 @@ cudaError_t ts_reduce_energy_diag(ts_ctx* c, int alpha, double* out_host);   // 
 cudaError_t ts_fill_basis(ts_ctx* c, uint64_t k);
 cudaError_t ts_fill_random_phase(ts_ctx* c, int up_spin, uint64_t seed);
 #define TS_TRACE_STRIDE (TS_MAX_N + 1)
-cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row /*[TS_TRACE_STRIDE]*/);
+cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row /*[TS_TRACE_STRIDE]*/, unsigned int* row_ctr = nullptr);
+cudaError_t ts_set_u32(ts_ctx* c, unsigned int* p, unsigned int v);

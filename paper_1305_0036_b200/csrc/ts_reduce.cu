@@ -323,6 +323,24 @@ __global__ void k_final_sum(const double* __restrict__ partial, int nblocks, int
     out[v] = s;
 }
 
+// the same into row *row_ctr of a trace (rows of TS_TRACE_STRIDE doubles), then *row_ctr += 1: a launch that can be replayed
+// from a CUDA graph and still fill consecutive rows (ts_evolve_observe)
+__global__ void k_final_sum_row(const double* __restrict__ partial, int nblocks, int nvals, double* __restrict__ base,
+                                unsigned int* __restrict__ row_ctr)
+{
+    const int v = threadIdx.x;
+    const unsigned int row = *row_ctr;
+    if (v < nvals) {
+        double s = 0.0;
+        for (int b = 0; b < nblocks; ++b) s += partial[(size_t)b * MAXV + v];
+        base[(size_t)row * TS_TRACE_STRIDE + v] = s;
+    }
+    __syncthreads();
+    if (v == 0) *row_ctr = row + 1;
+}
+
+__global__ void k_set_u32(unsigned int* p, unsigned int v) { *p = v; }
+
 __global__ void k_fill_basis(double2* __restrict__ psi, uint64_t dim, uint64_t kset)
 {
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
@@ -363,9 +381,10 @@ cudaError_t finish(ts_ctx* c, int grid, int nvals, double* host_out)
 }
 
 // final sum of nvals values into a DEVICE buffer, no copy, no synchronisation (observable traces)
-cudaError_t finish_dev(ts_ctx* c, int grid, int nvals, double* dev_out)
+cudaError_t finish_dev(ts_ctx* c, int grid, int nvals, double* dev_out, unsigned int* row_ctr)
 {
-    k_final_sum<<<1, 64, 0, c->stream>>>(c->d_red, grid, nvals, dev_out);
+    if (row_ctr) k_final_sum_row<<<1, 64, 0, c->stream>>>(c->d_red, grid, nvals, dev_out, row_ctr);
+    else k_final_sum<<<1, 64, 0, c->stream>>>(c->d_red, grid, nvals, dev_out);
     ts_prof_end(c);
     return cudaGetLastError();
 }
@@ -375,7 +394,15 @@ cudaError_t finish_dev(ts_ctx* c, int grid, int nvals, double* dev_out)
 // One row of an observable trace, written to device memory on the stream (ts_evolve_observe):
 // alpha = z: row[0] = <psi|psi>, row[1 + j] = sum_{k: bit j = 1} |c_k|^2 for all j;  alpha = x, y: row[0], row[1] = the
 // Re and Im pair sums of site j.  The host turns rows into expectation values after the single final copy.
-cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row)
+cudaError_t ts_set_u32(ts_ctx* c, unsigned int* p, unsigned int v)
+{
+    k_set_u32<<<1, 1, 0, c->stream>>>(p, v);
+    return cudaGetLastError();
+}
+
+// row_ctr = NULL: the row is written at dev_row.  Otherwise dev_row is the trace's first row and the row index is read from
+// (and then advanced in) *row_ctr on the device.
+cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row, unsigned int* row_ctr)
 {
     if (alpha == TS_Z) {
         const uint64_t dim = (uint64_t)1 << c->N;
@@ -385,7 +412,7 @@ cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row)
         ts_prof_begin(c, TS_KC_REDUCE);
         if (c->N >= 12) k_prob_bits_chunked<<<grid, RB, 0, c->stream>>>(c->psi, c->N, dim >> 12, c->d_red);
         else k_prob_bits<<<grid, RB, 0, c->stream>>>(c->psi, c->N, dim, c->d_red);
-        return finish_dev(c, grid, c->N + 1, dev_row);
+        return finish_dev(c, grid, c->N + 1, dev_row, row_ctr);
     }
     const uint64_t npairs = (uint64_t)1 << (c->N - 1);
     const int grid = red_grid(npairs);
@@ -393,7 +420,7 @@ cudaError_t ts_reduce_trace_row(ts_ctx* c, int alpha, int j, double* dev_row)
     if (e != cudaSuccess) return e;
     ts_prof_begin(c, TS_KC_REDUCE);
     k_pair_xy<<<grid, RB, 0, c->stream>>>(c->psi, j, npairs, c->d_red);
-    return finish_dev(c, grid, 2, dev_row);
+    return finish_dev(c, grid, 2, dev_row, row_ctr);
 }
 
 cudaError_t ts_reduce_expect_z_all(ts_ctx* c, double* out_host)

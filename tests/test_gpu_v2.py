@@ -414,3 +414,23 @@ def test_graph_replay_of_small_states(B, N, kernel, order):
     assert out[0][1] == out[1][1]                  # same number of kernel launches accounted
     assert np.array_equal(out[0][0], out[1][0])
     check_amps(out[0][0], oracle_run(w, steps, order))
+
+
+def test_evolve_observe_graph_replay_matches_launch_by_launch(B):
+    """ts_evolve_observe on a small state replays [one step + the row's reduction] from a CUDA graph, the row index
+    advancing on the device: same trace, bit for bit, as the launch-by-launch path, and against the oracle."""
+    N, steps = 15, 12
+    w = W.generic(N, seed=9100, tau=0.02, n_steps=steps)
+    traces = []
+    for graph in (1, 0):
+        ts = B.TrotterSuzuki(N, w.h, w.J)
+        ts.set_option(B.OPT_GRAPH, graph)
+        ts.set_state(w.state())
+        traces.append(ts.evolve_observe(w.tau, steps, 4, B.Z, -1))          # all sites, every step
+        assert ts.get_option(B.OPT_GRAPH_REPLAYS) == (steps - 1 if graph else 0)
+        ts.close()
+    assert np.array_equal(traces[0], traces[1])
+    psi = w.state()
+    for k in range(steps):
+        O.evolve(psi, N, w.h, w.J, w.tau, 1, 4, True)
+        assert np.max(np.abs(traces[0][k] - O.expect_all(psi, N, O.Z))) <= OBS_TOL
