@@ -225,6 +225,14 @@ const char* ts_version(void);
  *                     receives from rank rho') on the shard's stream or ordered with it, and return 0; it is called 20
  *                     times per 4th-order step (4 per 2nd-order step), an even number, so after the call the amplitudes
  *                     are again in layout 0 and in the buffer they started in.  g = 0: exchange may be NULL.
+ *   ts_shard_bind_peers  PEER-MEMORY MODE: bufs0[r], bufs1[r] = the two buffers of rank r (r < 2^g) as DEVICE pointers valid on
+ *                     this rank's device (peer-mapped over NVLink: CUDA IPC handles, or plain pointers when the ranks share
+ *                     a process or a device); entry [rank] must be this shard's own buffers.  The exchange and the pass over
+ *                     the arriving spins then run as ONE kernel that gathers its tiles from the peers' shards, and
+ *                     `exchange` is only called as a barrier, with src = dst = NULL: it must return once every rank's work
+ *                     queued so far is ordered before what this rank queues next (e.g. a 1-element all-reduce on the
+ *                     stream).  Needs shards of >= 13 spins whose top bit group has >= g bits, g <= 5.  NULL, NULL: back to
+ *                     the exchange mode.
  *   ts_shard_info     local spin count, current layout (0 / 1) and current buffer (0 / 1).
  *   ts_shard_spin_map spin_of_bit[N]: the spin on each local bit (first N-g entries), then on each rank bit, in `config`.
  *   ts_shard_ctx      the context of a layout: for the read-only calls (ts_expect_all, ts_norm2, ts_get_state) on this
@@ -235,6 +243,7 @@ typedef int (*ts_exchange_fn)(void* user, void* src_dev, void* dst_dev);
 int ts_shard_create(ts_shard** out, int N, const double* h, const double* J, int log2_ranks, int rank);
 int ts_shard_destroy(ts_shard* s);
 int ts_shard_bind(ts_shard* s, void* buf0_dev, void* buf1_dev);
+int ts_shard_bind_peers(ts_shard* s, const void* const* bufs0_dev, const void* const* bufs1_dev);
 int ts_shard_set_stream(ts_shard* s, void* cuda_stream);
 int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exchange_fn exchange, void* user);
 int ts_shard_info(ts_shard* s, int* n_local, int* config, int* buffer);

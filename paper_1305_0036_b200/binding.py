@@ -28,7 +28,7 @@ SYMBOLS = ("ts_create", "ts_destroy", "ts_set_stream", "ts_bind_state", "ts_set_
            "ts_describe_plan", "ts_set_profiling", "ts_get_profile", "ts_reset_profile", "ts_strerror", "ts_version",
            "ts_set_plan_groups", "ts_set_option", "ts_get_option", "ts_get_profile_passes", "ts_correlate", "ts_total_sz",
            "ts_energy", "ts_set_random_phase_state", "ts_loschmidt_echo", "ts_load_plan_file",
-           "ts_shard_create", "ts_shard_destroy", "ts_shard_bind", "ts_shard_set_stream", "ts_shard_evolve", "ts_shard_info",
+           "ts_shard_create", "ts_shard_destroy", "ts_shard_bind", "ts_shard_bind_peers", "ts_shard_set_stream", "ts_shard_evolve", "ts_shard_info",
            "ts_shard_spin_map", "ts_shard_ctx")
 
 _lib = None
@@ -85,6 +85,7 @@ def load() -> ctypes.CDLL:
         "ts_shard_create": (I, [ctypes.POINTER(_vp), I, _dp, _dp, I, I]),
         "ts_shard_destroy": (I, [_vp]),
         "ts_shard_bind": (I, [_vp, _vp, _vp]),
+        "ts_shard_bind_peers": (I, [_vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp)]),
         "ts_shard_set_stream": (I, [_vp, _vp]),
         "ts_shard_evolve": (I, [_vp, D, I64, I, EXCHANGE_FN, _vp]),
         "ts_shard_info": (I, [_vp, ctypes.POINTER(I), ctypes.POINTER(I), ctypes.POINTER(I)]),

@@ -144,6 +144,8 @@ void ts_tile_free_tables(ts_ctx* c);
 // which phase-table layout the pass (group, kind1, kind2) will use (0 / 1), i.e. which kernel family runs it
 int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2);
 cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d /*or NULL*/, int kind2);
+cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, const double2* const* peers, int gbits, int rank,
+                             double2* dst);
 bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb);
 // [H(gh) single ka] [A fused ka . D . kb] [H(gh) single kb] in one L2-blocked launch
 cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int kb);

@@ -24,7 +24,15 @@
 // copies between the shards of one GPU in the single-GPU test.  Everything else (sequence, rotations, diagonals) is this
 // library's own kernels.  Per sweep a shard makes one tile pass per bit group plus ONE pass that rotates the arriving spins
 // and applies the diagonal (the top group's pass restricted to its top g bits); fusing that pass with the next sweep's
-// top group and moving the exchange into the kernel over peer memory come next.
+// top group comes next.
+//
+// PEER-MEMORY MODE (ts_shard_bind_peers; NVLink 5 / NVSwitch gives every GPU load/store access to every peer's HBM): the
+// exchange and the pass over the arrivals are ONE kernel (k_tile_pass_p2p, ts_tile_kernel.cuh).  The arrival pass's tiles
+// are gathered straight from the peers' shards -- the rows whose top g row bits equal rho' are loaded from rank rho' at
+// the position that has this rank's number in those bits, which is exactly what the all-to-all would have delivered --
+// rotated, multiplied by the diagonal and stored into this rank's other buffer.  No collective moves data; what is left of
+// the callback is a barrier (src = dst = NULL): "every rank has finished its local sweep".  One barrier per sweep
+// suffices: a rank overwrites the buffer its peers read from only in its NEXT arrival pass, i.e. after the next barrier.
 #include <math.h>
 #include <string.h>
 
@@ -37,6 +45,7 @@ struct ts_shard {
     ts_ctx* cfg[2];
     double2* buf[2];
     int cur_cfg, cur_buf;
+    const double2* peer[2][256];     // peer-memory mode: buffer 0 / 1 of every rank as mapped into this device (else peer[0][0] = NULL)
 };
 
 namespace {
@@ -147,6 +156,7 @@ int ts_shard_create(ts_shard** out, int N, const double* h, const double* J, int
     if (!s) return TS_ERR_NOMEM;
     s->N = N; s->g = g; s->n = N - g; s->rank = rank;
     s->cfg[0] = s->cfg[1] = nullptr; s->buf[0] = s->buf[1] = nullptr; s->cur_cfg = 0; s->cur_buf = 0;
+    s->peer[0][0] = nullptr;
     int st = make_cfg(s, 0, h, J);
     if (st == TS_OK) st = make_cfg(s, 1, h, J);
     if (st != TS_OK) { ts_shard_destroy(s); return st; }
@@ -175,6 +185,23 @@ int ts_shard_bind(ts_shard* s, void* buf0, void* buf1)
     int st = ts_bind_state(s->cfg[0], buf0);
     if (st == TS_OK) st = ts_bind_state(s->cfg[1], buf0);
     return st;
+}
+
+int ts_shard_bind_peers(ts_shard* s, const void* const* bufs0, const void* const* bufs1)
+{
+    if (!s) return TS_ERR_ARG;
+    if (!bufs0 || !bufs1) { s->peer[0][0] = nullptr; return TS_OK; }          // back to the exchange callback
+    if (!s->buf[0] || s->g < 1 || s->g > 5) return TS_ERR_ARG;
+    // the arrival pass is the top bit group's tile pass: the shard must have one, with at least g bits
+    const ts_ctx* c = s->cfg[0];
+    if (c->groups.size() < 2 || TS_TILE_LOG2 - c->groups.back().s < s->g) return TS_ERR_ARG;
+    for (int r = 0; r < (1 << s->g); ++r) {
+        if (!bufs0[r] || !bufs1[r]) return TS_ERR_ARG;
+        s->peer[0][r] = (const double2*)bufs0[r];
+        s->peer[1][r] = (const double2*)bufs1[r];
+    }
+    if (s->peer[0][s->rank] != s->buf[0] || s->peer[1][s->rank] != s->buf[1]) { s->peer[0][0] = nullptr; return TS_ERR_ARG; }
+    return TS_OK;
 }
 
 int ts_shard_set_stream(ts_shard* s, void* stream)
@@ -235,7 +262,17 @@ int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exch
         case 2: d.alpha = TS_Y; d.t = 0.5 * su; d.scale_pow = -s->N; break;
         default: d.alpha = TS_Z; d.t = 0.5 * su + 0.5 * sub(u + 1); d.scale_pow = -s->N; break;
         }
-        if (s->g > 0) {
+        if (s->g > 0 && s->peer[0][0]) {
+            // peer-memory mode: barrier, then the arrival pass gathers its tiles from the peers' current buffers
+            if (exchange(user, nullptr, nullptr) != 0) return TS_ERR_CUDA;
+            double2* dst = s->buf[s->cur_buf ^ 1];
+            ts_ctx* cn = s->cfg[s->cur_cfg ^ 1];
+            ts_bind_state(cn, (void*)dst);
+            e = ts_tile_pass_p2p(cn, (int)cn->groups.size() - 1, kind, &d, s->peer[s->cur_buf], s->g, s->rank, dst);
+            s->cur_buf ^= 1; s->cur_cfg ^= 1;
+            ts_bind_state(s->cfg[0], (void*)dst);
+            ts_bind_state(s->cfg[1], (void*)dst);
+        } else if (s->g > 0) {
             double2* src = s->buf[s->cur_buf];
             double2* dst = s->buf[s->cur_buf ^ 1];
             if (exchange(user, (void*)src, (void*)dst) != 0) return TS_ERR_CUDA;

@@ -13,6 +13,7 @@
 namespace {
 
 tile_kernel_t g_tab[5][5];                 // k_tile_pass, run-time butterfly masks
+tile_kernel_t g_p2p[5];                    // k_tile_pass_p2p (sharded state vector: tiles gathered from peer memory)
 v2_kernel_t g_v2[3][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits
 v2_chunk_kernel_t g_v2_chunk[2][2];        // [9-bit high group][(Y^dag, Y), (X, X^dag)]
 v2_chunk_kernel_t g_probe_chunk[2];        // measurement builds (ts_v2_probe.cu): [arithmetic only, exchanges only]
@@ -185,6 +186,7 @@ void init_once()
 {
     memset(g_tab, 0, sizeof(g_tab));
     ts_tile_register_generic(&g_tab);
+    ts_tile_register_p2p(&g_p2p);
     memset(g_v2, 0, sizeof(g_v2));
     ts_v2_register_A(&g_v2[0]);
     ts_v2_register_Hf(&g_v2[1]);
@@ -222,6 +224,9 @@ void init_once()
             if (g_tab[k1][k2])
                 e = cudaFuncSetAttribute((const void*)g_tab[k1][k2], cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)(sizeof(double2) << TS_TILE_LOG2));
+    for (int k = 0; k < 5 && e == cudaSuccess; ++k)
+        if (g_p2p[k])
+            e = cudaFuncSetAttribute((const void*)g_p2p[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double2) << TS_TILE_LOG2));
     g_init_status = e;
 }
 
@@ -239,6 +244,8 @@ void fill_v1_params(const ts_ctx* c, const TileGroup& g, const DiagTables* tb, T
     } else {
         for (int r = 0; r < 32; ++r) p->RR[r] = make_double2(1.0, 0.0);
     }
+    for (int k = 0; k < 8; ++k) p->peers[k] = nullptr;
+    p->dst = nullptr; p->p2p_gbits = 0; p->p2p_rank = 0;
     p->s = g.s; p->g0 = g.g0;
     // butterflied bits: all of the group's, or (c->top_bits_only > 0) only its top `top_bits_only` ones; the layouts the
     // tile moves through -- and with them the diagonal's tables -- are those of the whole group either way
@@ -436,6 +443,32 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
     if (c->dry_run) return cudaSuccess;
     ts_prof_begin(c, fused ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
     k<<<(unsigned)ntiles, TS_TILE_THREADS, smem, c->stream>>>(p);
+    ts_prof_end(c);
+    return cudaGetLastError();
+}
+
+// Sharded state vector (ts_shard.cu): one sweep's butterflies on the top `gbits` bits of `group` (the spins that would have
+// arrived with the all-to-all) and the diagonal, the tiles gathered straight from the peers' shards.
+cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, const double2* const* peers, int gbits, int rank,
+                             double2* dst)
+{
+    const TileGroup& g = c->groups[group];
+    if (g.is_low || gbits < 1 || gbits > 5 || TS_TILE_LOG2 - g.s < gbits || !g_p2p[kind]) return cudaErrorInvalidValue;
+    const DiagTables* tb = nullptr;
+    if (d && d->present) {
+        cudaError_t e = ts_tile_get_tables(c, *d, group, 0, &tb);
+        if (e != cudaSuccess) return e;
+    }
+    TilePassParams p;
+    c->top_bits_only = gbits;
+    fill_v1_params(c, g, tb, &p);
+    c->top_bits_only = 0;
+    for (int k = 0; k < (1 << gbits); ++k) p.peers[k] = peers[k];
+    p.dst = dst; p.p2p_gbits = gbits; p.p2p_rank = rank;
+    const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
+    const size_t smem = p.two_stage ? (sizeof(double2) << TS_TILE_LOG2) : 0;
+    ts_prof_begin(c, TS_KC_TILE_SINGLE, 1.0);
+    g_p2p[kind]<<<(unsigned)ntiles, TS_TILE_THREADS, smem, c->stream>>>(p);
     ts_prof_end(c);
     return cudaGetLastError();
 }

@@ -12,3 +12,12 @@ void ts_tile_register_generic(tile_kernel_t (*tab)[5][5])
     G(SW_NONE, SW_NONE);
 #undef G
 }
+
+void ts_tile_register_p2p(tile_kernel_t (*tab)[5])
+{
+    (*tab)[SW_YDAG] = tsk::k_tile_pass_p2p<SW_YDAG>;
+    (*tab)[SW_Y] = tsk::k_tile_pass_p2p<SW_Y>;
+    (*tab)[SW_XDAG] = tsk::k_tile_pass_p2p<SW_XDAG>;
+    (*tab)[SW_X] = tsk::k_tile_pass_p2p<SW_X>;
+    (*tab)[SW_NONE] = nullptr;
+}

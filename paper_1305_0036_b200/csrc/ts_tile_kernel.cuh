@@ -49,12 +49,20 @@ struct TilePassParams {
     int nshfl;                   // 2 for group A, else 0                                  (generic kernel only)
     unsigned bf1, bf2;           // butterflied register bits in layout 1 / layout 2       (generic kernel only)
     double2 RR[32];              // read straight from the constant bank
+    // ---- peer-memory pass of a sharded state vector (k_tile_pass_p2p, ts_shard.cu): the tile's rows whose top `p2p_gbits`
+    // row bits equal rho are LOADED from peers[rho] -- rank rho's shard as mapped into this device, read over NVLink --
+    // at the position that has this rank's number in those bits (the all-to-all index-bit swap folded into the load), and
+    // the finished tile is stored to `dst` (this rank's other buffer).  Unused (gbits = 0) by the in-place passes.
+    const double2* peers[8];
+    double2* dst;
+    int p2p_gbits, p2p_rank;
 };
 
 typedef void (*tile_kernel_t)(const TilePassParams);
 
 // registry filled by ts_tile_cfgG.cu
 void ts_tile_register_generic(tile_kernel_t (*tab)[5][5]);
+void ts_tile_register_p2p(tile_kernel_t (*tab)[5]);      // [kind]: k_tile_pass_p2p
 
 #ifdef __CUDACC__
 namespace tsk {
@@ -170,7 +178,7 @@ __device__ __forceinline__ void apply_diag(const TilePassParams& p, double2 base
 
 // One tile: load (layout 1), sweep K1, diagonal, sweep K2, store in place.  CG bit 0: bypass L1 on the loads
 // (ld.global.cg); bit 1: keep the stores in L2 (st.global.cg) instead of streaming them out (st.global.cs).
-template <int K1, int K2, int BF1, int BF2, int NSHFL, int CG>
+template <int K1, int K2, int BF1, int BF2, int NSHFL, int CG, bool P2P = false>
 __device__ __forceinline__ void tile_body(const TilePassParams& p, const uint64_t tau, double2* sm)
 {
     constexpr bool GENERIC = (BF1 < 0);
@@ -196,13 +204,31 @@ __device__ __forceinline__ void tile_body(const TilePassParams& p, const uint64_
     double2* __restrict__ gp = p.psi + base_idx + offt;
 
     double re[32], im[32];
+    if (P2P) {
+        // register bits 5 - gbits .. 4 are the tile's top row bits: they name the peer the row comes from; in the peer's
+        // shard the row sits where those bits spell THIS rank
+        const int lowb = 5 - p.p2p_gbits;
+        uint64_t rank_off = 0;
 #pragma unroll
-    for (int r = 0; r < 32; ++r) {
-        uint64_t o = 0;
+        for (int b = 0; b < 5; ++b) if (b >= lowb && ((p.p2p_rank >> (b - lowb)) & 1)) rank_off |= offb[b];
+        const uint64_t toff = base_idx + offt + rank_off;
 #pragma unroll
-        for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
-        const double2 v = (CG & 1) ? __ldcg(gp + o) : __ldcs(gp + o);
-        re[r] = v.x; im[r] = v.y;
+        for (int r = 0; r < 32; ++r) {
+            uint64_t o = 0;
+#pragma unroll
+            for (int b = 0; b < 5; ++b) if ((r & (1 << b)) && b < lowb) o |= offb[b];
+            const double2 v = __ldcs(p.peers[r >> lowb] + toff + o);
+            re[r] = v.x; im[r] = v.y;
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            uint64_t o = 0;
+#pragma unroll
+            for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
+            const double2 v = (CG & 1) ? __ldcg(gp + o) : __ldcs(gp + o);
+            re[r] = v.x; im[r] = v.y;
+        }
     }
 
     // phase factors of this thread (loads overlap the data loads in flight)
@@ -235,13 +261,14 @@ __device__ __forceinline__ void tile_body(const TilePassParams& p, const uint64_
     }
     bfly_regs<K2, BF1>(re, im, p.bf1);
 
+    double2* __restrict__ sp = P2P ? (p.dst + base_idx + offt) : gp;
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
         uint64_t o = 0;
 #pragma unroll
         for (int b = 0; b < 5; ++b) if (r & (1 << b)) o |= offb[b];
-        if (CG & 2) __stcg(gp + o, make_double2(re[r], im[r]));
-        else __stcs(gp + o, make_double2(re[r], im[r]));
+        if (CG & 2) __stcg(sp + o, make_double2(re[r], im[r]));
+        else __stcs(sp + o, make_double2(re[r], im[r]));
     }
 }
 
@@ -250,6 +277,14 @@ __global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __gri
 {
     extern __shared__ double2 sm[];          // 4096 slots when layout 2 is used
     tile_body<K1, K2, BF1, BF2, NSHFL, 0>(p, p.tile_base + blockIdx.x, sm);
+}
+
+// One sweep's butterflies on the top p2p_gbits bits of the group (+ the diagonal), tiles gathered from peer memory.
+template <int K1>
+__global__ void __launch_bounds__(TS_TILE_THREADS, 2) k_tile_pass_p2p(const __grid_constant__ TilePassParams p)
+{
+    extern __shared__ double2 sm[];
+    tile_body<K1, SW_NONE, -1, -1, 0, 0, true>(p, p.tile_base + blockIdx.x, sm);
 }
 
 } // namespace tsk

@@ -6,7 +6,9 @@ The method's arithmetic (rotations, diagonals, their sequence, the effective Ham
   * `alltoall_exchange`: the once-per-sweep index-bit swap as `torch.distributed.all_to_all_single` (NCCL over NVLink /
     NVSwitch on GPUs; gloo in the CPU test): block rho' of a rank's shard goes to rank rho', block rho' of the result comes
     from rank rho';
-  * `ShardedTrotterSuzuki`: one rank's shard (two device buffers, the ts_shard object, the exchange callback);
+  * `ShardedTrotterSuzuki`: one rank's shard (two device buffers, the ts_shard object, the exchange callback); with
+    `bind_peers` (or `share_buffers_over_ipc` under torch.distributed) it runs in PEER-MEMORY MODE: the library's arrival
+    pass gathers its tiles straight from the peers' shards over NVLink and the callback shrinks to a barrier;
   * `LocalCluster`: all G shards of a small system on ONE GPU, one Python thread per rank, the exchange done by plain
     device copies between the shards -- how the sharded path is checked against the oracle on a single-GPU box;
   * index bookkeeping to scatter / gather a full state and to assemble <S^z_j> over ranks.
@@ -82,17 +84,59 @@ class ShardedTrotterSuzuki:
         B._check(self._lib.ts_shard_set_stream(self._s, B._vp(torch.cuda.current_stream(self.device).cuda_stream)),
                  "ts_shard_set_stream")
         self._exchange = exchange if exchange is not None else (lambda s, d: alltoall_exchange(s, d, group))
+        self._barrier = lambda: None
         self._error = None
         self._cb = B.EXCHANGE_FN(self._callback)       # keep the thunk alive as long as the shard
 
     def _callback(self, user, src, dst) -> int:
         try:
+            if not src:                                # peer-memory mode: only a barrier is asked for
+                self._barrier()
+                return 0
             k = 0 if src == self.buf[0].data_ptr() else 1
             self._exchange(self.buf[k], self.buf[k ^ 1])
             return 0
         except BaseException as exc:                   # never let an exception cross the C frame
             self._error = exc
             return 1
+
+    # ------------------------------------------------------------------ peer-memory mode
+    def bind_peers(self, ptrs0, ptrs1, barrier: Callable[[], None]) -> None:
+        """ptrs0[r], ptrs1[r]: device pointers (valid on this device) of rank r's two buffers; `barrier()` must order every
+        rank's queued work before what this rank queues next."""
+        a0 = (B._vp * self.world)(*[B._vp(int(p)) for p in ptrs0])
+        a1 = (B._vp * self.world)(*[B._vp(int(p)) for p in ptrs1])
+        B._check(self._lib.ts_shard_bind_peers(self._s, a0, a1), "ts_shard_bind_peers")
+        self._barrier = barrier
+
+    def share_buffers_over_ipc(self, group=None) -> None:
+        """Peer-memory mode under torch.distributed, one process per GPU of one node: every rank exports its two buffers as
+        CUDA IPC handles (torch's storage sharing), all-gathers them, maps the peers' buffers into its own address space and
+        hands the pointers to the library; the barrier is a one-element all-reduce on the stream.  (Written against the
+        torch 2.11 storage-sharing calls; no multi-GPU box was available to this build to run it on.)"""
+        import torch
+        import torch.distributed as dist
+        mine = [b.untyped_storage()._share_cuda_() for b in self.buf]
+        everyone = [None] * self.world
+        dist.all_gather_object(everyone, mine, group=group)
+        self._peer_keepalive = []
+        ptrs = [[], []]
+        for r, handles in enumerate(everyone):
+            for k in range(2):
+                if r == self.rank:
+                    ptrs[k].append(self.buf[k].data_ptr())
+                    continue
+                h = list(handles[k])
+                h[0] = self.device.index if self.device.index is not None else torch.cuda.current_device()
+                st = torch.UntypedStorage._new_shared_cuda(*h)
+                t = torch.empty(0, dtype=torch.complex128, device=self.device).set_(st)
+                self._peer_keepalive.append(t)
+                ptrs[k].append(t.data_ptr())
+        token = torch.zeros(1, device=self.device)
+
+        def barrier():
+            dist.all_reduce(token, group=group)
+        self.bind_peers(ptrs[0], ptrs[1], barrier)
 
     # ------------------------------------------------------------------ state
     def info(self):
@@ -168,7 +212,7 @@ class LocalCluster:
     the shards (all on the same stream, so stream order is the only synchronisation the data needs; the thread barrier
     makes sure every rank has issued its part of the sweep before anybody copies)."""
 
-    def __init__(self, N: int, h, J, world: int, device: str = "cuda:0"):
+    def __init__(self, N: int, h, J, world: int, device: str = "cuda:0", peer_memory: bool = False):
         import torch
         self._torch = torch
         self.N, self.world = int(N), int(world)
@@ -176,6 +220,13 @@ class LocalCluster:
         self._barrier = threading.Barrier(world)
         self._src: List = [None] * world
         self.shards = [ShardedTrotterSuzuki(N, h, J, r, world, device, exchange=self._make_exchange(r)) for r in range(world)]
+        if peer_memory:
+            # every "peer" buffer lives on this GPU: plain pointers.  All ranks launch into the same stream, so the thread
+            # barrier (everybody has QUEUED its local sweep) is all the ordering the gather needs.
+            p0 = [s.buf[0].data_ptr() for s in self.shards]
+            p1 = [s.buf[1].data_ptr() for s in self.shards]
+            for s in self.shards:
+                s.bind_peers(p0, p1, lambda: self._barrier.wait(timeout=120))
 
     def _make_exchange(self, r: int):
         def exchange(src, dst):

@@ -26,11 +26,11 @@ def S():
     return sharded
 
 
-def run_case(S, N, world, order, steps, seed, symmetric_fill=False):
+def run_case(S, N, world, order, steps, seed, symmetric_fill=False, peer_memory=False):
     w = W.generic(N, seed=seed, tau=0.02, n_steps=steps, symmetric_fill=symmetric_fill)
     ref = w.state()
     O.evolve(ref, N, w.h, w.J, w.tau, steps, order, True)
-    cl = S.LocalCluster(N, w.h, w.J, world)
+    cl = S.LocalCluster(N, w.h, w.J, world, peer_memory=peer_memory)
     cl.set_state(w.state())
     cl.evolve(w.tau, steps, order)
     got = cl.get_state()
@@ -56,6 +56,22 @@ def test_sharded_with_multi_group_shards(S, N, world):
     """Shards of 19 / 20 spins: several bit groups per shard, a two-stage top group, and the arriving spins rotated by
     the top group's tile pass restricted to its top g bits (fused with the diagonal)."""
     run_case(S, N, world, 4, steps=1, seed=4700 + N)
+
+
+# shards of >= 13 spins (the arrival pass is the top bit group's tile pass); single- and two-stage top groups, g = 1, 2, 3
+@pytest.mark.parametrize("N,world", [(14, 2), (15, 2), (16, 4), (17, 4), (19, 8), (20, 4), (22, 8)])
+@pytest.mark.parametrize("order", [4, 2])
+def test_peer_memory_mode_matches_full_oracle(S, N, world, order):
+    """Peer-memory mode: no exchange; the arrival pass gathers its tiles from the other shards' buffers (here: plain
+    pointers on the same GPU; across GPUs: peer-mapped pointers) and writes into the shard's other buffer."""
+    run_case(S, N, world, order, steps=2 if N <= 20 else 1, seed=4800 + 10 * N + world, peer_memory=True)
+
+
+def test_peer_memory_mode_needs_a_top_group(S):
+    from paper_1305_0036_b200 import binding as B
+    w = W.generic(10, seed=3, tau=0.01, n_steps=1)
+    with pytest.raises(B.TSError):
+        S.LocalCluster(10, w.h, w.J, 4, peer_memory=True)        # shards of 8 spins have no tile groups
 
 
 def test_one_rank_is_the_unsharded_path(S):
