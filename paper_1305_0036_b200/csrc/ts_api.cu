@@ -873,7 +873,7 @@ int ts_total_sz(ts_ctx* c, double* out)
 
 // One global rotation (sweep) of the state, optionally followed by the exact scaling 2^scale_pow: every group of the
 // plan once (tiled), or one launch per spin (naive / small-N contexts).
-cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow)
+cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow, int skip_last_group)
 {
     cudaError_t e = cudaSuccess;
     DiagOp d; d.present = (scale_pow != 0); d.alpha = TS_Z; d.t = 0.0; d.scale_pow = scale_pow;
@@ -882,7 +882,7 @@ cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow)
         if (e == cudaSuccess && d.present) e = ts_naive_diag(c, d);
         return e;
     }
-    const int g = (int)c->groups.size();
+    const int g = (int)c->groups.size() - (skip_last_group ? 1 : 0);      // (skipped: done by a fused pass before)
     for (int gi = 0; gi < g && e == cudaSuccess; ++gi)
         e = ts_tile_pass(c, gi, kind, (gi == g - 1 && d.present) ? &d : nullptr, SW_NONE);
     return e;

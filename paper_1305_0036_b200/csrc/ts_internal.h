@@ -87,7 +87,7 @@ struct ts_ctx {
     int opt_l2_hints;                    // L2 eviction priorities on the TMA transfers of the L2-blocked launch
     int opt_graph;                       // 1: small states replay one step's launches from a CUDA graph (ts_api.cu)
     int opt_graph_max_n;                 // largest N that does so
-    int top_bits_only;                   // > 0 (transient, ts_shard.cu): a high-group pass butterflies only its top so-many bits
+    int top_bits_only;                   // > 0 (transient, ts_shard.cu): a high-group pass's FIRST sweep butterflies only the group's top so-many bits
     int dry_run;                         // launchers build / look up their phase tables and return without launching
     cudaGraphExec_t g_exec;              // the graph of the last graph-mode ts_evolve call (released lazily, after g_done)
     cudaEvent_t g_done;
@@ -126,7 +126,7 @@ void ts_prof_end(ts_ctx* c);
 
 // One global rotation (sweep) of the whole local state, optionally followed by the exact scaling 2^scale_pow: every group
 // of the plan once (tiled), or one launch per spin (ts_api.cu).
-cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow);
+cudaError_t ts_apply_sweep_all(ts_ctx* c, int kind, int scale_pow, int skip_last_group = 0);
 
 // ---- naive path (ts_naive.cu)
 cudaError_t ts_naive_rotate(ts_ctx* c, int j, int kind);
@@ -144,8 +144,8 @@ void ts_tile_free_tables(ts_ctx* c);
 // which phase-table layout the pass (group, kind1, kind2) will use (0 / 1), i.e. which kernel family runs it
 int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2);
 cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d /*or NULL*/, int kind2);
-cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, const double2* const* peers, int gbits, int rank,
-                             double2* dst);
+cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, int kind2, const double2* const* peers, int gbits,
+                             int rank, double2* dst);
 bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb);
 // [H(gh) single ka] [A fused ka . D . kb] [H(gh) single kb] in one L2-blocked launch
 cudaError_t ts_tile_chunk_triple(ts_ctx* c, int gh, int ka, const DiagOp& d, int kb);

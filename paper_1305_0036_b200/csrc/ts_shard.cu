@@ -22,9 +22,9 @@
 // The exchange itself is the caller's: a callback that moves 2^n amplitudes from `src` to `dst` (both device buffers on
 // this rank) through whatever joins the ranks -- NCCL all-to-all over NVLink in paper_1305_0036_b200/sharded.py, plain
 // copies between the shards of one GPU in the single-GPU test.  Everything else (sequence, rotations, diagonals) is this
-// library's own kernels.  Per sweep a shard makes one tile pass per bit group plus ONE pass that rotates the arriving spins
-// and applies the diagonal (the top group's pass restricted to its top g bits); fusing that pass with the next sweep's
-// top group comes next.
+// library's own kernels.  Per sweep a shard makes one tile pass per bit group: the top group's pass is the ARRIVAL pass,
+// [sweep i on the g arrived spins] . D_i . [sweep i+1 on the whole top group] (its first sweep restricted to the group's top
+// g bits), so sweep i+1's local passes start below it.
 //
 // PEER-MEMORY MODE (ts_shard_bind_peers; NVLink 5 / NVSwitch gives every GPU load/store access to every peer's HBM): the
 // exchange and the pass over the arrivals are ONE kernel (k_tile_pass_p2p, ts_tile_kernel.cuh).  The arrival pass's tiles
@@ -93,31 +93,30 @@ int make_cfg(ts_shard* s, int cfg, const double* h, const double* J)
     return TS_OK;
 }
 
-// rotation `kind` on local spins [first, first + count) of a context: all of them -> one tile pass per bit group;
-// otherwise one launch per spin (the g spins that arrive with an exchange)
-cudaError_t rotate_range(ts_ctx* c, int kind, int first, int count)
+// The whole local sweep of a context: one tile pass per bit group (the top one left out when the previous arrival pass has
+// done it already), or one launch per spin for shards below 12 spins.
+cudaError_t local_sweep(ts_ctx* c, int kind, bool top_group_done)
 {
-    if (count <= 0) return cudaSuccess;
-    if (first == 0 && count == c->N) return ts_apply_sweep_all(c, kind, 0);
-    cudaError_t e = cudaSuccess;
-    for (int j = first; j < first + count && e == cudaSuccess; ++j) e = ts_naive_rotate(c, j, kind);
-    return e;
+    return ts_apply_sweep_all(c, kind, 0, top_group_done ? 1 : 0);
+}
+
+// Can the arrival pass be the top bit group's tile pass?  (A shard of >= 13 spins whose top group has at least g bits.)
+bool arrival_is_a_tile_pass(const ts_ctx* c, int g)
+{
+    return c->groups.size() >= 2 && TS_TILE_LOG2 - c->groups.back().s >= g;
 }
 
 // The g spins that arrived with an exchange sit on the top g local bits, i.e. on the top bits of the plan's last bit
-// group: their rotation and the diagonal that follows the sweep are ONE tile pass of that group restricted to those bits.
-// (Shards below 12 spins, or a top group with fewer than g bits: one launch per spin, then the diagonal.)
-cudaError_t rotate_arrivals_then_diagonal(ts_ctx* c, int kind, int g, const DiagOp& d)
+// group: their rotation (sweep `kind`), the diagonal that follows the sweep and the NEXT sweep's butterflies on the whole
+// group (`kind2`, SW_NONE after the last sweep) are ONE tile pass of that group.  (Shards below 13 spins, or a top group
+// with fewer than g bits: one launch per spin, then the diagonal; kind2 must be SW_NONE.)
+cudaError_t rotate_arrivals_then_diagonal(ts_ctx* c, int kind, int g, const DiagOp& d, int kind2)
 {
-    if (!c->groups.empty() && c->groups.size() >= 2) {
-        const int last = (int)c->groups.size() - 1;
-        const TileGroup& tg = c->groups[last];
-        if (TS_TILE_LOG2 - tg.s >= g) {
-            c->top_bits_only = g;
-            cudaError_t e = ts_tile_pass(c, last, kind, d.present ? &d : nullptr, SW_NONE);
-            c->top_bits_only = 0;
-            return e;
-        }
+    if (arrival_is_a_tile_pass(c, g)) {
+        c->top_bits_only = g;
+        cudaError_t e = ts_tile_pass(c, (int)c->groups.size() - 1, kind, d.present ? &d : nullptr, kind2);
+        c->top_bits_only = 0;
+        return e;
     }
     cudaError_t e = cudaSuccess;
     for (int j = c->N - g; j < c->N && e == cudaSuccess; ++j) e = ts_naive_rotate(c, j, kind);
@@ -250,9 +249,12 @@ int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exch
     cudaError_t e = cudaSuccess;
     DiagOp d; d.present = 1; d.alpha = TS_Z; d.t = 0.5 * sub(0); d.scale_pow = 0;
     e = diagonal(s->cfg[s->cur_cfg], d);
+    const bool fuse = s->g > 0 && arrival_is_a_tile_pass(s->cfg[0], s->g);
+    bool top_done = false;               // the top group's butterflies of this sweep were done by the last arrival pass
     for (int64_t i = 1; i <= M && e == cudaSuccess; ++i) {
         const int kind = kinds[(i - 1) & 3];
-        e = rotate_range(s->cfg[s->cur_cfg], kind, 0, s->n);
+        const int kind2 = (fuse && i < M) ? kinds[i & 3] : SW_NONE;
+        e = local_sweep(s->cfg[s->cur_cfg], kind, top_done);
         if (e != cudaSuccess) break;
         const int64_t u = (i - 1) >> 2;
         const double su = sub(u);
@@ -268,10 +270,11 @@ int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exch
             double2* dst = s->buf[s->cur_buf ^ 1];
             ts_ctx* cn = s->cfg[s->cur_cfg ^ 1];
             ts_bind_state(cn, (void*)dst);
-            e = ts_tile_pass_p2p(cn, (int)cn->groups.size() - 1, kind, &d, s->peer[s->cur_buf], s->g, s->rank, dst);
+            e = ts_tile_pass_p2p(cn, (int)cn->groups.size() - 1, kind, &d, kind2, s->peer[s->cur_buf], s->g, s->rank, dst);
             s->cur_buf ^= 1; s->cur_cfg ^= 1;
             ts_bind_state(s->cfg[0], (void*)dst);
             ts_bind_state(s->cfg[1], (void*)dst);
+            top_done = (kind2 != SW_NONE);
         } else if (s->g > 0) {
             double2* src = s->buf[s->cur_buf];
             double2* dst = s->buf[s->cur_buf ^ 1];
@@ -279,7 +282,8 @@ int ts_shard_evolve(ts_shard* s, double tau, int64_t n_steps, int order, ts_exch
             s->cur_buf ^= 1; s->cur_cfg ^= 1;
             ts_bind_state(s->cfg[0], (void*)dst);
             ts_bind_state(s->cfg[1], (void*)dst);
-            e = rotate_arrivals_then_diagonal(s->cfg[s->cur_cfg], kind, s->g, d);
+            e = rotate_arrivals_then_diagonal(s->cfg[s->cur_cfg], kind, s->g, d, kind2);
+            top_done = (kind2 != SW_NONE);
         } else {
             e = diagonal(s->cfg[s->cur_cfg], d);
         }

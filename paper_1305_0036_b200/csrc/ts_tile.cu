@@ -13,7 +13,7 @@
 namespace {
 
 tile_kernel_t g_tab[5][5];                 // k_tile_pass, run-time butterfly masks
-tile_kernel_t g_p2p[5];                    // k_tile_pass_p2p (sharded state vector: tiles gathered from peer memory)
+tile_kernel_t g_p2p[5][5];                 // k_tile_pass_p2p (sharded state vector: tiles gathered from peer memory)
 v2_kernel_t g_v2[3][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits
 v2_chunk_kernel_t g_v2_chunk[2][2];        // [9-bit high group][(Y^dag, Y), (X, X^dag)]
 v2_chunk_kernel_t g_probe_chunk[2];        // measurement builds (ts_v2_probe.cu): [arithmetic only, exchanges only]
@@ -186,6 +186,7 @@ void init_once()
 {
     memset(g_tab, 0, sizeof(g_tab));
     ts_tile_register_generic(&g_tab);
+    memset(g_p2p, 0, sizeof(g_p2p));
     ts_tile_register_p2p(&g_p2p);
     memset(g_v2, 0, sizeof(g_v2));
     ts_v2_register_A(&g_v2[0]);
@@ -224,9 +225,11 @@ void init_once()
             if (g_tab[k1][k2])
                 e = cudaFuncSetAttribute((const void*)g_tab[k1][k2], cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)(sizeof(double2) << TS_TILE_LOG2));
-    for (int k = 0; k < 5 && e == cudaSuccess; ++k)
-        if (g_p2p[k])
-            e = cudaFuncSetAttribute((const void*)g_p2p[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double2) << TS_TILE_LOG2));
+    for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
+        for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
+            if (g_p2p[k1][k2])
+                e = cudaFuncSetAttribute((const void*)g_p2p[k1][k2], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)(sizeof(double2) << TS_TILE_LOG2));
     g_init_status = e;
 }
 
@@ -252,9 +255,13 @@ void fill_v1_params(const ts_ctx* c, const TileGroup& g, const DiagTables* tb, T
     const int nb = (c->top_bits_only > 0 && !g.is_low) ? c->top_bits_only : n_bfly(g);
     p->two_stage = two_stage(g) ? 1 : 0;
     p->nshfl = g.is_low ? 2 : 0;
-    if (g.is_low) { p->bf1 = 31u; p->bf2 = 31u; }
-    else if (nb <= 5) { p->bf1 = (31u << (5 - nb)) & 31u; p->bf2 = 0u; }          // top nb bits of f 7..11 (layout 1)
-    else { p->bf1 = 31u; p->bf2 = (31u << (10 - nb)) & 31u; }                       // top nb-5 bits of f 2..6
+    auto masks = [&](int bits, unsigned& m1, unsigned& m2) {
+        if (g.is_low) { m1 = 31u; m2 = 31u; }
+        else if (bits <= 5) { m1 = (31u << (5 - bits)) & 31u; m2 = 0u; }          // top `bits` bits of f 7..11 (layout 1)
+        else { m1 = 31u; m2 = (31u << (10 - bits)) & 31u; }                        // + top bits-5 bits of f 2..6
+    };
+    masks(nb, p->bf1, p->bf2);
+    masks(n_bfly(g), p->bf1b, p->bf2b);       // a second sweep in the same pass always takes all of the group's bits
 }
 
 void fill_v2_geom(const TileGroup& g, V2Geom* q, int top_bits_only = 0)
@@ -395,6 +402,7 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
     // automatic choice: the persistent pipeline pays once every SM walks several tiles; with at most two tiles per SM
     // (N <= 20 on 148 SMs) the one-CTA-per-tile kernel is faster (no pipeline set-up: 283 vs 361 us per step at N = 20)
     if (c->opt_kernel == 2 && (((uint64_t)1 << (c->N - TS_TILE_LOG2)) <= 2ull * (uint64_t)c->num_sms)) return 0;
+    if (c->top_bits_only > 0 && !g.is_low && kind2 != SW_NONE) return 0;   // separate masks per sweep: k_tile_pass only
     return g_v2[(c->top_bits_only > 0 && !g.is_low) ? 1 : v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
@@ -447,13 +455,14 @@ cudaError_t ts_tile_pass(ts_ctx* c, int group, int kind1, const DiagOp* d, int k
     return cudaGetLastError();
 }
 
-// Sharded state vector (ts_shard.cu): one sweep's butterflies on the top `gbits` bits of `group` (the spins that would have
-// arrived with the all-to-all) and the diagonal, the tiles gathered straight from the peers' shards.
-cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, const double2* const* peers, int gbits, int rank,
-                             double2* dst)
+// Sharded state vector (ts_shard.cu): sweep `kind`'s butterflies on the top `gbits` bits of `group` (the spins that would
+// have arrived with the all-to-all), the diagonal, and sweep `kind2`'s butterflies on all of the group's bits (SW_NONE: none),
+// the tiles gathered straight from the peers' shards.
+cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, int kind2, const double2* const* peers, int gbits,
+                             int rank, double2* dst)
 {
     const TileGroup& g = c->groups[group];
-    if (g.is_low || gbits < 1 || gbits > 5 || TS_TILE_LOG2 - g.s < gbits || !g_p2p[kind]) return cudaErrorInvalidValue;
+    if (g.is_low || gbits < 1 || gbits > 5 || TS_TILE_LOG2 - g.s < gbits || !g_p2p[kind][kind2]) return cudaErrorInvalidValue;
     const DiagTables* tb = nullptr;
     if (d && d->present) {
         cudaError_t e = ts_tile_get_tables(c, *d, group, 0, &tb);
@@ -467,8 +476,8 @@ cudaError_t ts_tile_pass_p2p(ts_ctx* c, int group, int kind, const DiagOp* d, co
     p.dst = dst; p.p2p_gbits = gbits; p.p2p_rank = rank;
     const uint64_t ntiles = (uint64_t)1 << (c->N - TS_TILE_LOG2);
     const size_t smem = p.two_stage ? (sizeof(double2) << TS_TILE_LOG2) : 0;
-    ts_prof_begin(c, TS_KC_TILE_SINGLE, 1.0);
-    g_p2p[kind]<<<(unsigned)ntiles, TS_TILE_THREADS, smem, c->stream>>>(p);
+    ts_prof_begin(c, kind2 != SW_NONE ? TS_KC_TILE_FUSED : TS_KC_TILE_SINGLE, 1.0);
+    g_p2p[kind][kind2]<<<(unsigned)ntiles, TS_TILE_THREADS, smem, c->stream>>>(p);
     ts_prof_end(c);
     return cudaGetLastError();
 }

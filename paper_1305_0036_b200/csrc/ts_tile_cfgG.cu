@@ -13,11 +13,10 @@ void ts_tile_register_generic(tile_kernel_t (*tab)[5][5])
 #undef G
 }
 
-void ts_tile_register_p2p(tile_kernel_t (*tab)[5])
+void ts_tile_register_p2p(tile_kernel_t (*tab)[5][5])
 {
-    (*tab)[SW_YDAG] = tsk::k_tile_pass_p2p<SW_YDAG>;
-    (*tab)[SW_Y] = tsk::k_tile_pass_p2p<SW_Y>;
-    (*tab)[SW_XDAG] = tsk::k_tile_pass_p2p<SW_XDAG>;
-    (*tab)[SW_X] = tsk::k_tile_pass_p2p<SW_X>;
-    (*tab)[SW_NONE] = nullptr;
+#define P(K1, K2) (*tab)[K1][K2] = tsk::k_tile_pass_p2p<K1, K2>
+    P(SW_XDAG, SW_YDAG); P(SW_YDAG, SW_Y); P(SW_Y, SW_X); P(SW_X, SW_XDAG);        // sweep i's arrivals . D_i . sweep i+1
+    P(SW_YDAG, SW_NONE); P(SW_Y, SW_NONE); P(SW_XDAG, SW_NONE); P(SW_X, SW_NONE);  // the last sweep of a call
+#undef P
 }

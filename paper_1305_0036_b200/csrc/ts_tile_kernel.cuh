@@ -47,7 +47,8 @@ struct TilePassParams {
     int s, g0;
     int two_stage;               // layout 2 is used (more than 5 butterflied bits)     (generic kernel only)
     int nshfl;                   // 2 for group A, else 0                                  (generic kernel only)
-    unsigned bf1, bf2;           // butterflied register bits in layout 1 / layout 2       (generic kernel only)
+    unsigned bf1, bf2;           // butterflied register bits in layout 1 / layout 2, sweep K1   (generic kernel only)
+    unsigned bf1b, bf2b;         // the same for sweep K2 (equal to bf1, bf2 except in a sharded sweep's arrival pass)
     double2 RR[32];              // read straight from the constant bank
     // ---- peer-memory pass of a sharded state vector (k_tile_pass_p2p, ts_shard.cu): the tile's rows whose top `p2p_gbits`
     // row bits equal rho are LOADED from peers[rho] -- rank rho's shard as mapped into this device, read over NVLink --
@@ -62,7 +63,7 @@ typedef void (*tile_kernel_t)(const TilePassParams);
 
 // registry filled by ts_tile_cfgG.cu
 void ts_tile_register_generic(tile_kernel_t (*tab)[5][5]);
-void ts_tile_register_p2p(tile_kernel_t (*tab)[5]);      // [kind]: k_tile_pass_p2p
+void ts_tile_register_p2p(tile_kernel_t (*tab)[5][5]);   // [k1][k2]: k_tile_pass_p2p
 
 #ifdef __CUDACC__
 namespace tsk {
@@ -256,10 +257,10 @@ __device__ __forceinline__ void tile_body(const TilePassParams& p, const uint64_
     // ---- sweep K2 (mirror order)
     if (two_stage) {
         if (nshfl) { bfly_lane<K2>(re, im, 1, lane); bfly_lane<K2>(re, im, 0, lane); }
-        bfly_regs<K2, BF2>(re, im, p.bf2);
+        bfly_regs<K2, BF2>(re, im, p.bf2b);
         exchange<false>(sm, re, im, t);
     }
-    bfly_regs<K2, BF1>(re, im, p.bf1);
+    bfly_regs<K2, BF1>(re, im, p.bf1b);
 
     double2* __restrict__ sp = P2P ? (p.dst + base_idx + offt) : gp;
 #pragma unroll
@@ -279,12 +280,13 @@ __global__ void __launch_bounds__(TS_TILE_THREADS, MINB) k_tile_pass(const __gri
     tile_body<K1, K2, BF1, BF2, NSHFL, 0>(p, p.tile_base + blockIdx.x, sm);
 }
 
-// One sweep's butterflies on the top p2p_gbits bits of the group (+ the diagonal), tiles gathered from peer memory.
-template <int K1>
+// Sweep K1's butterflies on the top p2p_gbits bits of the group, the diagonal, then sweep K2's butterflies on ALL of the
+// group's bits (the next sweep starts with this group); tiles gathered from peer memory.
+template <int K1, int K2>
 __global__ void __launch_bounds__(TS_TILE_THREADS, 2) k_tile_pass_p2p(const __grid_constant__ TilePassParams p)
 {
     extern __shared__ double2 sm[];
-    tile_body<K1, SW_NONE, -1, -1, 0, 0, true>(p, p.tile_base + blockIdx.x, sm);
+    tile_body<K1, K2, -1, -1, 0, 0, true>(p, p.tile_base + blockIdx.x, sm);
 }
 
 } // namespace tsk
