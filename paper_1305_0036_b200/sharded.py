@@ -272,3 +272,47 @@ class LocalCluster:
     def close(self) -> None:
         for s in self.shards:
             s.close()
+
+
+def _main(argv=None) -> int:
+    """`python -m paper_1305_0036_b200.sharded --N 28 --world 4 [--peer-memory]`: time the sharded path with all shards on ONE
+    GPU (LocalCluster) next to the single-context path -- what the sharding costs in local work, exchange included as
+    device copies; it says nothing about NVLink."""
+    import argparse
+    import json
+    import time
+    import torch
+    from . import workloads as W
+    ap = argparse.ArgumentParser(description=_main.__doc__)
+    ap.add_argument("--N", type=int, default=28)
+    ap.add_argument("--world", type=int, default=4)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--peer-memory", action="store_true")
+    a = ap.parse_args(argv)
+    w = W.grid_like(a.N, seed=8, tau=0.01, n_steps=1, state_seed=9, cols=6 if a.N >= 24 else None)
+    ts = B.TrotterSuzuki(a.N, w.h, w.J)
+    ts.set_random_phase_state(0, seed=9)
+    ts.evolve(w.tau, 1, 4)
+    torch.cuda.synchronize()
+    t = time.perf_counter()
+    ts.evolve(w.tau, a.steps, 4)
+    torch.cuda.synchronize()
+    one = (time.perf_counter() - t) / a.steps
+    ts.close()
+    del ts
+    torch.cuda.empty_cache()
+    cl = LocalCluster(a.N, w.h, w.J, a.world, peer_memory=a.peer_memory)
+    for s in cl.shards:
+        s.buf[0].fill_(2.0 ** (-a.N / 2.0))
+    cl.evolve(w.tau, 1, 4)
+    t = time.perf_counter()
+    cl.evolve(w.tau, a.steps, 4)
+    sh = (time.perf_counter() - t) / a.steps
+    print(json.dumps({"N": a.N, "shards_on_one_gpu": a.world, "peer_memory": a.peer_memory, "single_context_ms_per_step": one * 1e3,
+                      "sharded_ms_per_step": sh * 1e3, "ratio": sh / one, "norm2_after": cl.norm2()}))
+    cl.close()
+    return 0
+
+
+if __name__ == "__main__":
+    raise SystemExit(_main())
