@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libts_b200.so")
-SOURCES = ["ts_v2_probe.cu", "ts_v2_chunk0.cu", "ts_v2_chunk1.cu", "ts_v2_chunk0_h9.cu", "ts_v2_chunk1_h9.cu", "ts_v2_H9.cu", "ts_v2_A.cu", "ts_v2_Hs.cu", "ts_v2_Hf.cu", "ts_tile_cfgG.cu", "ts_api.cu", "ts_shard.cu",
+SOURCES = ["ts_v2_probe.cu", "ts_v2_chunk0.cu", "ts_v2_chunk1.cu", "ts_v2_chunk0_h9.cu", "ts_v2_chunk1_h9.cu", "ts_v2_H9.cu", "ts_v2_H10.cu", "ts_v2_A.cu", "ts_v2_Hs.cu", "ts_v2_Hf.cu", "ts_tile_cfgG.cu", "ts_api.cu", "ts_shard.cu",
            "ts_tile.cu", "ts_naive.cu", "ts_small.cu", "ts_reduce.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("TS_EXTRA_NVCC", "").split()

@@ -90,7 +90,13 @@ int build_plan(ts_ctx* c)
         int mgmax = TS_TILE_LOG2 - s_min;
         if (c->max_group_bits > 0 && c->max_group_bits < mgmax) mgmax = c->max_group_bits;
         int left = rem;
-        if (c->run_bits == 0 && c->max_group_bits == 0 && rem > mgmax) {
+        if (c->run_bits == 0 && c->max_group_bits == 0 && rem == 2 * (mgmax + 1)) {
+            // N = 32: two groups of TEN bits (64-byte runs, no L2-blocked launch: the chunk would be 64 MiB) beat 9 + 6 + 5
+            // with its extra tile pass per sweep: 1 272 vs 1 392 ms per step (profiles/r02_ab_and_sizes.md)
+            bits.push_back(mgmax + 1);
+            bits.push_back(mgmax + 1);
+            left = 0;
+        } else if (c->run_bits == 0 && c->max_group_bits == 0 && rem > mgmax) {
             // default plan: the group right above A takes as many bits as a pass can (9), so that A + that group is a
             // 32-MiB chunk the L2-blocked triple launch keeps on chip (ts_tile_v2.cuh) at every N >= 22 ...
             bits.push_back(mgmax);
@@ -100,7 +106,7 @@ int build_plan(ts_ctx* c)
         // many for a single group (N = 31) is still ONE group, with 64-byte runs: measured 597 vs 673 ms per step against
         // two groups of five (profiles/r02_ab_and_sizes.md) -- a tile pass more per sweep costs more than short runs do.
         const bool ten = (c->run_bits == 0 && c->max_group_bits == 0 && left == mgmax + 1);
-        const int ng = ten ? 1 : (left + mgmax - 1) / mgmax;
+        const int ng = left == 0 ? 0 : ten ? 1 : (left + mgmax - 1) / mgmax;
         for (int i = 0; i < ng; ++i) bits.push_back(left / ng + (i < left % ng ? 1 : 0));
     }
     int g0 = TS_TILE_LOG2;

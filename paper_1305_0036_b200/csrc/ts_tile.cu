@@ -14,7 +14,7 @@ namespace {
 
 tile_kernel_t g_tab[5][5];                 // k_tile_pass, run-time butterfly masks
 tile_kernel_t g_p2p[5][5];                 // k_tile_pass_p2p (sharded state vector: tiles gathered from peer memory)
-v2_kernel_t g_v2[3][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits
+v2_kernel_t g_v2[4][5][5];                 // [type][k1][k2]: group A, high group (run-time masks), high group of 9 bits, of 10 bits
 v2_chunk_kernel_t g_v2_chunk[2][2];        // [9-bit high group][(Y^dag, Y), (X, X^dag)]
 v2_chunk_kernel_t g_probe_chunk[2];        // measurement builds (ts_v2_probe.cu): [arithmetic only, exchanges only]
 v2_kernel_t g_probe_H[2], g_probe_A[2];
@@ -35,9 +35,9 @@ struct PhaseGeom {
 inline int spin_of_fbit(const TileGroup& g, int f) { return f < g.s ? f : g.g0 + (f - g.s); }
 inline int n_bfly(const TileGroup& g) { return g.is_low ? TS_TILE_LOG2 : TS_TILE_LOG2 - g.s; }
 inline bool two_stage(const TileGroup& g) { return n_bfly(g) > 5; }
-inline bool v2_geometry_ok(const TileGroup& g) { return g.is_low || (g.s >= 3 && g.s <= 11); }
+inline bool v2_geometry_ok(const TileGroup& g) { return g.is_low || (g.s >= 2 && g.s <= 11); }   // s = 2: the ten-bit kernels
 inline int nib(uint32_t pack, int i) { return (int)((pack >> (4 * i)) & 15u); }
-inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : 1); }     // kernel table index
+inline int v2_type(const TileGroup& g) { return g.is_low ? 0 : (g.s == 3 ? 2 : (g.s == 2 ? 3 : 1)); }     // kernel table index
 
 // layout 0: k_tile_pass.  layout 1: v2 (ts_tile_v2.cuh: the diagonal is applied in A2', H2 or H1).
 PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
@@ -55,8 +55,9 @@ PhaseGeom make_geom(const ts_ctx* c, const TileGroup& g, double t, int layout)
             q.tspin[b] = spin_of_fbit(g, f);
         }
     } else {
-        const uint32_t RP = g.is_low ? TS_V2_A2S_R : (two ? TS_V2_H2_R : TS_V2_H1_R);
-        const uint32_t TP = g.is_low ? TS_V2_A2S_T : (two ? TS_V2_H2_T : TS_V2_H1_T);
+        const bool ten = (!g.is_low && g.s == 2);
+        const uint32_t RP = g.is_low ? TS_V2_A2S_R : ten ? TS_V2_H2X_R : (two ? TS_V2_H2_R : TS_V2_H1_R);
+        const uint32_t TP = g.is_low ? TS_V2_A2S_T : ten ? TS_V2_H2X_T : (two ? TS_V2_H2_T : TS_V2_H1_T);
         for (int b = 0; b < 5; ++b) q.rspin[b] = spin_of_fbit(g, nib(RP, b));
         for (int b = 0; b < 7; ++b) q.tspin[b] = spin_of_fbit(g, nib(TP, b));
     }
@@ -194,6 +195,7 @@ void init_once()
     ts_v2_register_Hs(&g_v2[1]);
     ts_v2_register_H9f(&g_v2[2]);
     ts_v2_register_H9s(&g_v2[2]);
+    ts_v2_register_H10(&g_v2[3]);
     memset(g_v2_chunk, 0, sizeof(g_v2_chunk));
     ts_v2_register_chunk0(g_v2_chunk);
     ts_v2_register_chunk1(g_v2_chunk);
@@ -206,7 +208,7 @@ void init_once()
     if (e == cudaSuccess && (qr != cudaDriverEntryPointSuccess || !fn)) e = cudaErrorNotSupported;
     if (e != cudaSuccess) { g_init_status = e; return; }
     g_encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
-    for (int ty = 0; ty < 3 && e == cudaSuccess; ++ty)
+    for (int ty = 0; ty < 4 && e == cudaSuccess; ++ty)
         for (int k1 = 0; k1 < 5 && e == cudaSuccess; ++k1)
             for (int k2 = 0; k2 < 5 && e == cudaSuccess; ++k2)
                 if (g_v2[ty][k1][k2])
@@ -270,6 +272,8 @@ void fill_v2_geom(const TileGroup& g, V2Geom* q, int top_bits_only = 0)
     q->s = g.s; q->g0 = g.g0;
     q->m = g.is_low ? 0 : TS_TILE_LOG2 - g.s;
     q->nmid = g.g0 - g.s;
+    q->unit_log2 = g.s < 3 ? g.s : 3;
+    q->box_rows_log2 = (q->m - 1 < 8) ? q->m - 1 : 8;
     q->two_stage = (!g.is_low && q->m > 5) ? 1 : 0;
     q->mask1 = 0u; q->mask2 = 0u;
     if (!g.is_low) {
@@ -315,14 +319,17 @@ cudaError_t v2_tensor_map(ts_ctx* c, int group, CUtensorMap* out)
         } else {
             const int m = TS_TILE_LOG2 - g.s;
             const int top = c->N - g.g0 - m;                     // index bits above the group
-            cuuint64_t dims[4] = {16, (cuuint64_t)1 << (g.g0 - 3), (cuuint64_t)1 << m, (cuuint64_t)1 << top};
-            cuuint64_t strides[3] = {128, (cuuint64_t)16 << g.g0, (cuuint64_t)16 << (g.g0 + m)};
-            cuuint32_t box[4] = {16, (cuuint32_t)1 << (g.s - 3), (cuuint32_t)1 << (m - 1), 1};
+            const int u = g.s < 3 ? g.s : 3;                     // unit = 2^u amplitudes (128 bytes; 64 for runs of 4)
+            const int rows_log2 = (m - 1 < 8) ? m - 1 : 8;       // a box dimension cannot exceed 256
+            cuuint64_t dims[4] = {(cuuint64_t)2 << u, (cuuint64_t)1 << (g.g0 - u), (cuuint64_t)1 << m, (cuuint64_t)1 << top};
+            cuuint64_t strides[3] = {(cuuint64_t)16 << u, (cuuint64_t)16 << g.g0, (cuuint64_t)16 << (g.g0 + m)};
+            cuuint32_t box[4] = {(cuuint32_t)2 << u, (cuuint32_t)1 << (g.s - u), (cuuint32_t)1 << rows_log2, 1};
             const CUtensorMapL2promotion prom = c->opt_l2_promotion == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
                                               : c->opt_l2_promotion == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
                                                                          : CU_TENSOR_MAP_L2_PROMOTION_NONE;
             r = g_encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)c->psi, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, prom, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, g.s < 3 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B, prom,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         }
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
         memcpy(sl.bytes, &tm, sizeof(tm));
@@ -402,7 +409,7 @@ int ts_tile_layout_for(const ts_ctx* c, int group, int kind1, int kind2)
     // automatic choice: the persistent pipeline pays once every SM walks several tiles; with at most two tiles per SM
     // (N <= 20 on 148 SMs) the one-CTA-per-tile kernel is faster (no pipeline set-up: 283 vs 361 us per step at N = 20)
     if (c->opt_kernel == 2 && (((uint64_t)1 << (c->N - TS_TILE_LOG2)) <= 2ull * (uint64_t)c->num_sms)) return 0;
-    if (c->top_bits_only > 0 && !g.is_low && kind2 != SW_NONE) return 0;   // separate masks per sweep: k_tile_pass only
+    if (c->top_bits_only > 0 && !g.is_low && (kind2 != SW_NONE || g.s < 3)) return 0;   // separate masks per sweep: k_tile_pass only
     return g_v2[(c->top_bits_only > 0 && !g.is_low) ? 1 : v2_type(g)][kind1][kind2] ? 1 : 0;
 }
 
@@ -488,7 +495,7 @@ bool ts_tile_chunk_supported(const ts_ctx* c, int gh, int ka, int kb)
     if (c->opt_chunk == 0 || c->opt_kernel == 0 || gh != 1 || (int)c->groups.size() < 3 || !c->groups[0].is_low) return false;
     if (ts_tile_layout_for(c, 0, ka, kb) == 0) return false;           // the TMA kernels are not in use at this size
     const TileGroup& g = c->groups[gh];
-    if (g.g0 != TS_TILE_LOG2 || !v2_geometry_ok(g)) return false;     // the group right above A
+    if (g.g0 != TS_TILE_LOG2 || !v2_geometry_ok(g) || g.s < 3) return false;     // the group right above A, 128-byte runs
     const int C = g.g0 + (TS_TILE_LOG2 - g.s);                         // chunk = spins 0 .. C-1
     if (C >= c->N || C > c->opt_chunk_max_log2) return false;          // at least two chunks, each small enough for L2
     if (C < c->opt_chunk_min_log2) return false;                       // small chunks: the hand-overs cost more than the round trips

@@ -30,6 +30,7 @@
 // register / thread bit):
 //   A1: regs {3,4,5,10,11}  threads {0,1,2,8,9,6,7}        A2: regs {0,1,2,8,9}  threads {3,4,5,6,7,10,11}
 //   H1: regs {7,8,9,10,11}  threads {0,1,2,3,4,5,6}        H2: regs {3,4,5,6,7}  threads {0,1,2,8,9,10,11}
+//   H1x: regs {5,8,9,10,11} threads {0,1,2,3,4,6,7}        H2x: regs {2,3,4,6,7} threads {0,1,5,8,9,10,11}   (ten-bit group)
 // Group A butterflies all 12 bits without warp shuffles: K1 on 5 bits in A1, 5 in A2, then A2 -> A2' (regs {0,1,2,6,7}:
 // lane bits 3, 4 swapped with register bits 3, 4 -- an exchange INSIDE each warp's quarter of the buffer, __syncwarp only)
 // and f6, f7 there; the diagonal in A2'; K2 on all five register bits of A2', the five of A1, and f8, f9 in A1'.  A high group butterflies f >= s: f7..11 in H1 and f_s..6 in H2 (m > 5 only; diagonal in H2, else H1).
@@ -67,12 +68,20 @@
 #define TS_V2_H1_T 0x6543210u
 #define TS_V2_H2_R 0x76543u
 #define TS_V2_H2_T 0xBA98210u
+// a high group of TEN bits (runs of 4 amplitudes = 64 bytes, TMA's 64-byte swizzle): two full five-bit stages, f2 .. f11.
+// (H1x is conflict-free under that swizzle; H2x, with f2 on a register bit, has two-way bank conflicts -- the LSU has the room)
+#define TS_V2_H1X_R 0xBA985u
+#define TS_V2_H1X_T 0x7643210u
+#define TS_V2_H2X_R 0x76432u
+#define TS_V2_H2X_T 0xBA98510u
 
 // One tile group as the kernel sees it.
 struct V2Geom {
     int type;               // 0: group A (contiguous tile), 1: high group
     int s, g0, m;           // high group: run bits, first spin, group bits (A: 12, 12, 0)
     int nmid;               // g0 - s: tile-index bits below the group
+    int unit_log2;          // amplitudes per tensor-map unit (inner box dimension): min(3, s), i.e. 128 or 64 bytes
+    int box_rows_log2;      // rows per TMA box: min(8, m - 1); a tile is 2^(m - box_rows_log2) boxes
     int two_stage;          // high group with m > 5: layouts H1 and H2
     unsigned mask1, mask2;  // butterflied register bits in H1 / H2
 };
@@ -109,12 +118,13 @@ struct V2Chunk {
 typedef void (*v2_kernel_t)(const V2Pass, const CUtensorMap);
 typedef void (*v2_chunk_kernel_t)(const V2Chunk, const CUtensorMap, const CUtensorMap);
 
-// tab[type][k1][k2]; type 0: group A, 1: high group (run-time masks), 2: high group with 9 group bits
+// tab[type][k1][k2]; type 0: group A, 1: high group (run-time masks), 2: high group with 9 group bits, 3: with 10
 void ts_v2_register_A(v2_kernel_t (*tab)[5][5]);
 void ts_v2_register_Hf(v2_kernel_t (*tab)[5][5]);
 void ts_v2_register_Hs(v2_kernel_t (*tab)[5][5]);
 void ts_v2_register_H9f(v2_kernel_t (*tab)[5][5]);
 void ts_v2_register_H9s(v2_kernel_t (*tab)[5][5]);
+void ts_v2_register_H10(v2_kernel_t (*tab)[5][5]);
 // tab[hm][v]: hm = 0: any high group, 1: 9 group bits;  v = 0: (Y^dag, Y), v = 1: (X, X^dag) -- the two kind pairs that
 // meet at group A in the sweep order
 void ts_v2_register_chunk0(v2_chunk_kernel_t (*tab)[2]);
@@ -244,7 +254,8 @@ __device__ __forceinline__ unsigned int v2_ld_acquire(const unsigned int* p)
 
 // ------------------------------------------------------------------------------------------------ register layouts
 // RP / TP: the f bit of register bit i / thread bit i, one nibble each.
-template <uint32_t RP, uint32_t TP>
+// SWZ: 7 = TMA's 128-byte swizzle (slot = f ^ (f >> 3 & 7), rows of 128 bytes), 3 = its 64-byte swizzle (rows of 64 bytes)
+template <uint32_t RP, uint32_t TP, uint32_t SWZ = 7u>
 struct V2Layout {
     // byte offset (within a tile buffer) of the slot of the thread part of f
     static __device__ __forceinline__ uint32_t thread_off(int t)
@@ -252,13 +263,13 @@ struct V2Layout {
         uint32_t f = 0;
 #pragma unroll
         for (int i = 0; i < 7; ++i) f |= (uint32_t)((t >> i) & 1) << ((TP >> (4 * i)) & 15u);
-        return (f ^ ((f >> 3) & 7u)) << 4;
+        return (f ^ ((f >> 3) & SWZ)) << 4;
     }
     static __host__ __device__ constexpr uint32_t reg_slot(int r)
     {
         uint32_t f = 0;
         for (int i = 0; i < 5; ++i) f |= (uint32_t)((r >> i) & 1) << ((RP >> (4 * i)) & 15u);
-        return f ^ ((f >> 3) & 7u);
+        return f ^ ((f >> 3) & SWZ);
     }
     // slot(f_t | f_r) = slot(f_t) ^ slot(f_r) (the swizzle is linear over bits); only the three low slot bits mix
     static __device__ __forceinline__ double2* ptr(unsigned char* buf, uint32_t toff, int r)
@@ -395,11 +406,12 @@ __device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, c
                                           const double2* tab, const int t, const int grp)
 {
     constexpr bool AR = (MODE & 1) != 0, EX = (MODE & 2) != 0;
-    using L1 = V2Layout<TS_V2_H1_R, TS_V2_H1_T>;
-    using L2 = V2Layout<TS_V2_H2_R, TS_V2_H2_T>;
+    constexpr bool TEN = (M == 10);                    // ten group bits: layouts H1x / H2x, all five register bits in both
+    using L1 = V2Layout<TEN ? TS_V2_H1X_R : TS_V2_H1_R, TEN ? TS_V2_H1X_T : TS_V2_H1_T, TEN ? 3u : 7u>;
+    using L2 = V2Layout<TEN ? TS_V2_H2X_R : TS_V2_H2_R, TEN ? TS_V2_H2X_T : TS_V2_H2_T, TEN ? 3u : 7u>;
     constexpr bool CT = (M > 0);
-    constexpr int MK1 = CT ? (int)v2_h_mask1(M > 0 ? M : 1) : -1;
-    constexpr int MK2 = CT ? (int)v2_h_mask2(M > 0 ? M : 1) : -1;
+    constexpr int MK1 = TEN ? 31 : (CT ? (int)v2_h_mask1(M > 0 ? M : 1) : -1);
+    constexpr int MK2 = TEN ? 31 : (CT ? (int)v2_h_mask2(M > 0 ? M : 1) : -1);
     const uint32_t o1 = L1::thread_off(t), o2 = L2::thread_off(t);
     const bool two = EX && (CT ? (M > 5) : (g.two_stage != 0));
     double re[32], im[32];
@@ -433,67 +445,56 @@ __device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, c
 
 // ------------------------------------------------------------------------------------------------ TMA issue
 // Tensor maps (ts_tile.cu): group A: the state as [2^(N-3)] rows of 16 doubles, box {16, 256}; high group: the state as
-// [top][2^m rows][2^(g0-3) units][16 doubles], box {16, 2^(s-3), 2^(m-1), 1}.  Two boxes (f bit 11 = 0 / 1) per tile.
-__device__ __forceinline__ void v2_tile_coords(const V2Geom& g, const uint64_t tile, int& c1, int& c2lo, int& c2hi, int& c3)
+// [top][2^m rows][2^(g0-u) units][2^(u+1) doubles] with u = unit_log2, box {2^(u+1), 2^(s-u), 2^box_rows_log2, 1}: a tile
+// is 2 (m <= 9) or 4 (m = 10) boxes of consecutive rows, landing one after the other.
+struct V2Boxes { int c1, c3, nbox, rows, bytes; };
+__device__ __forceinline__ V2Boxes v2_tile_boxes(const V2Geom& g, const uint64_t tile)
 {
-    if (g.type == 0) {
-        c1 = (int)(tile << 9); c2lo = 0; c2hi = 256; c3 = 0;          // (2-D: row = c1 + c2)
-    } else {
+    V2Boxes b;
+    if (g.type == 0) { b.c1 = (int)(tile << 9); b.c3 = 0; b.nbox = 2; b.rows = 256; b.bytes = 32768; }
+    else {
         const uint64_t mid = tile & (((uint64_t)1 << g.nmid) - 1);
-        c1 = (int)(mid << (g.s - 3));
-        c2lo = 0; c2hi = 1 << (g.m - 1);
-        c3 = (int)(tile >> g.nmid);
+        b.c1 = (int)(mid << (g.s - g.unit_log2));
+        b.c3 = (int)(tile >> g.nmid);
+        b.rows = 1 << g.box_rows_log2;
+        b.nbox = 1 << (g.m - g.box_rows_log2);
+        b.bytes = TS_V2_TILE_BYTES >> (g.m - g.box_rows_log2);
     }
+    return b;
 }
 __device__ __forceinline__ void v2_issue_load(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t dst,
                                               const uint32_t bar)
 {
-    int c1, c2lo, c2hi, c3;
-    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
-    if (g.type == 0) {
-        v2_tma_load_2d(dst, tm, bar, 0, c1 + c2lo);
-        v2_tma_load_2d(dst + 32768u, tm, bar, 0, c1 + c2hi);
-    } else {
-        v2_tma_load_4d(dst, tm, bar, 0, c1, c2lo, c3);
-        v2_tma_load_4d(dst + 32768u, tm, bar, 0, c1, c2hi, c3);
+    const V2Boxes b = v2_tile_boxes(g, tile);
+    for (int q = 0; q < b.nbox; ++q) {
+        if (g.type == 0) v2_tma_load_2d(dst + q * b.bytes, tm, bar, 0, b.c1 + q * b.rows);
+        else v2_tma_load_4d(dst + q * b.bytes, tm, bar, 0, b.c1, q * b.rows, b.c3);
     }
 }
 __device__ __forceinline__ void v2_issue_load_h(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t dst,
                                                 const uint32_t bar, const uint64_t pol)
 {
-    int c1, c2lo, c2hi, c3;
-    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
-    if (g.type == 0) {
-        v2_tma_load_2d_h(dst, tm, bar, 0, c1 + c2lo, pol);
-        v2_tma_load_2d_h(dst + 32768u, tm, bar, 0, c1 + c2hi, pol);
-    } else {
-        v2_tma_load_4d_h(dst, tm, bar, 0, c1, c2lo, c3, pol);
-        v2_tma_load_4d_h(dst + 32768u, tm, bar, 0, c1, c2hi, c3, pol);
+    const V2Boxes b = v2_tile_boxes(g, tile);
+    for (int q = 0; q < b.nbox; ++q) {
+        if (g.type == 0) v2_tma_load_2d_h(dst + q * b.bytes, tm, bar, 0, b.c1 + q * b.rows, pol);
+        else v2_tma_load_4d_h(dst + q * b.bytes, tm, bar, 0, b.c1, q * b.rows, b.c3, pol);
     }
 }
 __device__ __forceinline__ void v2_issue_store_h(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src,
                                                  const uint64_t pol)
 {
-    int c1, c2lo, c2hi, c3;
-    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
-    if (g.type == 0) {
-        v2_tma_store_2d_h(tm, src, 0, c1 + c2lo, pol);
-        v2_tma_store_2d_h(tm, src + 32768u, 0, c1 + c2hi, pol);
-    } else {
-        v2_tma_store_4d_h(tm, src, 0, c1, c2lo, c3, pol);
-        v2_tma_store_4d_h(tm, src + 32768u, 0, c1, c2hi, c3, pol);
+    const V2Boxes b = v2_tile_boxes(g, tile);
+    for (int q = 0; q < b.nbox; ++q) {
+        if (g.type == 0) v2_tma_store_2d_h(tm, src + q * b.bytes, 0, b.c1 + q * b.rows, pol);
+        else v2_tma_store_4d_h(tm, src + q * b.bytes, 0, b.c1, q * b.rows, b.c3, pol);
     }
 }
 __device__ __forceinline__ void v2_issue_store(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src)
 {
-    int c1, c2lo, c2hi, c3;
-    v2_tile_coords(g, tile, c1, c2lo, c2hi, c3);
-    if (g.type == 0) {
-        v2_tma_store_2d(tm, src, 0, c1 + c2lo);
-        v2_tma_store_2d(tm, src + 32768u, 0, c1 + c2hi);
-    } else {
-        v2_tma_store_4d(tm, src, 0, c1, c2lo, c3);
-        v2_tma_store_4d(tm, src + 32768u, 0, c1, c2hi, c3);
+    const V2Boxes b = v2_tile_boxes(g, tile);
+    for (int q = 0; q < b.nbox; ++q) {
+        if (g.type == 0) v2_tma_store_2d(tm, src + q * b.bytes, 0, b.c1 + q * b.rows);
+        else v2_tma_store_4d(tm, src + q * b.bytes, 0, b.c1, q * b.rows, b.c3);
     }
 }
 
@@ -556,7 +557,8 @@ __device__ __forceinline__ void v2_push_end(unsigned char* smraw, const uint32_t
 }
 
 // ------------------------------------------------------------------------------------------------ one tile pass
-// TYPE 0: group A, 1: high group (any m), 2: high group with m = 9 (masks folded).  MODE: see v2_body_A.
+// TYPE 0: group A, 1: high group (any m <= 9), 2: high group with m = 9 (masks folded), 3: high group with m = 10 (64-byte
+// runs, layouts H1x / H2x).  MODE: see v2_body_A.
 template <int TYPE, int K1, int K2, int MODE = 3>
 __global__ void __launch_bounds__(TS_V2_THREADS, 1)
 k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap tmap)
@@ -630,6 +632,7 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
                 const double2* tp = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TP + b * 512u);
                 if constexpr (TYPE == 0) v2_body_A<K1, K2, MODE>(buf, has_diag, scale, tp, tab, t, grp);
                 else if constexpr (TYPE == 2) v2_body_H<K1, K2, 9, MODE>(buf, p.g, has_diag, scale, tp, tab, t, grp);
+                else if constexpr (TYPE == 3) v2_body_H<K1, K2, 10, MODE>(buf, p.g, has_diag, scale, tp, tab, t, grp);
                 else v2_body_H<K1, K2, -1, MODE>(buf, p.g, has_diag, scale, tp, tab, t, grp);
                 v2_fence_async_smem();                 // my shared-memory writes -> visible to the TMA store
             }

@@ -106,7 +106,7 @@ def test_default_plan_N24_triple_launch_three_steps(B, family):
     ts.close()
 
 
-@pytest.mark.parametrize("N,groups", [(18, [3, 3]), (22, [9, 1]), (21, [9]), (19, [4, 3]), (22, [5, 5])])
+@pytest.mark.parametrize("N,groups", [(18, [3, 3]), (22, [9, 1]), (21, [9]), (19, [4, 3]), (22, [5, 5]), (23, [10, 1])])
 def test_kernel_families_agree_and_match_oracle(B, N, groups):
     """The same plan through (a) the v2 kernels with the triple launch, (b) v2 without it, (c) the one-CTA-per-tile
     kernels: each against the oracle."""
