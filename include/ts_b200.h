@@ -144,7 +144,7 @@ int ts_set_plan(ts_ctx* ctx, int mode, int run_bits, int max_group_bits);
 
 /* Explicit plan: the number of index bits of every high group, bottom to top (group k butterflies the high_bits[k]
  * spins above group k-1; group A = spins 0..11 is implied).  sum(high_bits) must be N - 12, each entry in [1, 11];
- * entries <= 9 (runs of >= 128 bytes) run on the pipelined kernels.  This is what the tuner
+ * entries <= 10 (runs of >= 64 bytes; 9 = the 128-byte runs of P:165-167) run on the pipelined TMA kernels.  This is what the tuner
  * (paper_1305_0036_b200/tuner.py; "a brute force search for the fastest series of rotations ... stored in a
  * file") searches over and what a stored plan file sets.  N >= 12 only.  Errors: TS_ERR_ARG. */
 int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);

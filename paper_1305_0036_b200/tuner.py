@@ -22,7 +22,7 @@ from typing import Iterable, List, Sequence, Tuple
 
 import numpy as np
 
-MAX_GROUP_BITS = 9          # runs of >= 128 bytes: the pipelined kernels' range
+MAX_GROUP_BITS = 10         # runs of >= 64 bytes: 9 bits = 128-byte runs, 10 bits = 64-byte runs (ts_v2_H10.cu)
 
 
 def compositions(total: int, max_part: int = MAX_GROUP_BITS, max_parts: int = 4) -> Iterable[Tuple[int, ...]]:
@@ -51,11 +51,13 @@ def candidates(N: int, max_groups: int = 4, max_splits: int = 12) -> List[dict]:
     if comps:
         gmin = min(len(c) for c in comps)
         comps = [c for c in comps if len(c) <= gmin + 1]
-        comps.sort(key=lambda c: (len(c), -c[0] if c else 0, max(c) if c else 0))
+        # most promising first: fewest groups, a full 9-bit group above A (the 32-MiB chunk of the L2-blocked launch), then
+        # the largest first group, then the longest shortest run
+        comps.sort(key=lambda c: (len(c), 0 if (c and c[0] == 9) else 1, -c[0] if c else 0, max(c) if c else 0))
         comps = comps[:max_splits]
     out = []
     for groups in comps:
-        chunk_possible = len(groups) >= 2 and 12 + groups[0] <= 21
+        chunk_possible = len(groups) >= 2 and groups[0] <= 9 and 12 + groups[0] <= 21
         for chunk in ((1, 0) if chunk_possible else (0,)):
             for kernel in (1,):          # the warp-specialised TMA kernels (ts_tile_v2.cuh)
                 out.append({"groups": list(groups), "chunk": chunk, "l2_promotion": 0, "kernel": kernel})
