@@ -48,7 +48,12 @@
 #define TS_V2_TILE_BYTES 65536
 #define TS_V2_OFF_TP (TS_V2_NBUF * TS_V2_TILE_BYTES)         // 3 x 512 B tile-phase records
 #define TS_V2_OFF_BAR (TS_V2_OFF_TP + TS_V2_NBUF * 512)      // full[3], done[3], free[3], tab mbarriers (80 B), then tile[3] (u32)
-#define TS_V2_OFF_TILE (TS_V2_OFF_BAR + 96)                  // tile index of the job in each buffer (written by the loader)
+#define TS_V2_OFF_TILE (TS_V2_OFF_BAR + 112)                 // tile index of the job in each buffer (written by the loader)
+// mbarriers (8 bytes each): full[3], done[3], free[3][half 0], free[3][half 1], tab
+#define TS_V2_BAR_FULL(b) (8u * (b))
+#define TS_V2_BAR_DONE(b) (8u * (TS_V2_NBUF + (b)))
+#define TS_V2_BAR_FREE(b, h) (8u * ((2 + (h)) * TS_V2_NBUF + (b)))
+#define TS_V2_BAR_TABLE (8u * 4 * TS_V2_NBUF)
 #define TS_V2_END 0xffffffffu                                // "no more tiles" marker in a tile slot
 #define TS_V2_OFF_TAB (TS_V2_OFF_BAR + 128)                  // per-launch phase tables: TT[128], WT[5][128], RR[32]
 #define TS_V2_TAB_BYTES (800 * 16)
@@ -236,6 +241,7 @@ __device__ __forceinline__ void v2_tma_store_4d_h(const CUtensorMap* tm, uint32_
 }
 __device__ __forceinline__ void v2_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void v2_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void v2_store_wait_read_but_one() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 __device__ __forceinline__ void v2_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void v2_fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void v2_fence_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
@@ -462,37 +468,39 @@ __device__ __forceinline__ V2Boxes v2_tile_boxes(const V2Geom& g, const uint64_t
     }
     return b;
 }
+// `half` 0 / 1: the boxes of the first / second half of the tile (a buffer is refilled half by half, see the loader)
 __device__ __forceinline__ void v2_issue_load(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t dst,
-                                              const uint32_t bar)
+                                              const uint32_t bar, const int half)
 {
     const V2Boxes b = v2_tile_boxes(g, tile);
-    for (int q = 0; q < b.nbox; ++q) {
+    for (int q = half * (b.nbox >> 1); q < (half + 1) * (b.nbox >> 1); ++q) {
         if (g.type == 0) v2_tma_load_2d(dst + q * b.bytes, tm, bar, 0, b.c1 + q * b.rows);
         else v2_tma_load_4d(dst + q * b.bytes, tm, bar, 0, b.c1, q * b.rows, b.c3);
     }
 }
 __device__ __forceinline__ void v2_issue_load_h(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t dst,
-                                                const uint32_t bar, const uint64_t pol)
+                                                const uint32_t bar, const uint64_t pol, const int half)
 {
     const V2Boxes b = v2_tile_boxes(g, tile);
-    for (int q = 0; q < b.nbox; ++q) {
+    for (int q = half * (b.nbox >> 1); q < (half + 1) * (b.nbox >> 1); ++q) {
         if (g.type == 0) v2_tma_load_2d_h(dst + q * b.bytes, tm, bar, 0, b.c1 + q * b.rows, pol);
         else v2_tma_load_4d_h(dst + q * b.bytes, tm, bar, 0, b.c1, q * b.rows, b.c3, pol);
     }
 }
 __device__ __forceinline__ void v2_issue_store_h(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src,
-                                                 const uint64_t pol)
+                                                 const uint64_t pol, const int half)
 {
     const V2Boxes b = v2_tile_boxes(g, tile);
-    for (int q = 0; q < b.nbox; ++q) {
+    for (int q = half * (b.nbox >> 1); q < (half + 1) * (b.nbox >> 1); ++q) {
         if (g.type == 0) v2_tma_store_2d_h(tm, src + q * b.bytes, 0, b.c1 + q * b.rows, pol);
         else v2_tma_store_4d_h(tm, src + q * b.bytes, 0, b.c1, q * b.rows, b.c3, pol);
     }
 }
-__device__ __forceinline__ void v2_issue_store(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src)
+__device__ __forceinline__ void v2_issue_store(const V2Geom& g, const CUtensorMap* tm, const uint64_t tile, const uint32_t src,
+                                               const int half)
 {
     const V2Boxes b = v2_tile_boxes(g, tile);
-    for (int q = 0; q < b.nbox; ++q) {
+    for (int q = half * (b.nbox >> 1); q < (half + 1) * (b.nbox >> 1); ++q) {
         if (g.type == 0) v2_tma_store_2d(tm, src + q * b.bytes, 0, b.c1 + q * b.rows);
         else v2_tma_store_4d(tm, src + q * b.bytes, 0, b.c1, q * b.rows, b.c3);
     }
@@ -513,11 +521,12 @@ __device__ __forceinline__ void v2_wait_full(const uint32_t bar_full, const uint
 __device__ __forceinline__ void v2_init_barriers(const uint32_t sBar)
 {
     for (int k = 0; k < TS_V2_NBUF; ++k) {
-        v2_mbar_init(sBar + 8 * k, 1);                                // full: the loader's expect_tx arrive
-        v2_mbar_init(sBar + 8 * (TS_V2_NBUF + k), TS_TILE_THREADS);   // done: every thread of the compute group
-        v2_mbar_init(sBar + 8 * (2 * TS_V2_NBUF + k), 1);             // free: the storer
+        v2_mbar_init(sBar + TS_V2_BAR_FULL(k), 2);                    // full: the loader's two expect_tx arrives (one per half)
+        v2_mbar_init(sBar + TS_V2_BAR_DONE(k), TS_TILE_THREADS);      // done: every thread of the compute group
+        v2_mbar_init(sBar + TS_V2_BAR_FREE(k, 0), 1);                 // free: the storer, once per half
+        v2_mbar_init(sBar + TS_V2_BAR_FREE(k, 1), 1);
     }
-    v2_mbar_init(sBar + 8 * 3 * TS_V2_NBUF, 1);                       // tab: the launch's thread tables have landed
+    v2_mbar_init(sBar + TS_V2_BAR_TABLE, 1);                          // tab: the launch's thread tables have landed
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     v2_fence_async_smem();
 }
@@ -550,9 +559,13 @@ __device__ __forceinline__ void v2_push_end(unsigned char* smraw, const uint32_t
 {
     for (int k = 0; k < 2; ++k, ++j) {
         const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-        if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
+        if (use > 0) {
+            v2_mbar_wait(sBar + TS_V2_BAR_FREE(b, 0), (use - 1) & 1u);
+            v2_mbar_wait(sBar + TS_V2_BAR_FREE(b, 1), (use - 1) & 1u);
+        }
         v2_st_tile(smraw, b, TS_V2_END);
-        v2_mbar_arrive(sBar + 8 * b);
+        v2_mbar_arrive(sBar + TS_V2_BAR_FULL(b));
+        v2_mbar_arrive(sBar + TS_V2_BAR_FULL(b));
     }
 }
 
@@ -579,8 +592,8 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
         v2_regs_dec<TS_V2_REGS_PRODUCER>();
         if (warp == 8 && (threadIdx.x & 31) == 0) {    // ---- loader
             if (has_diag) {
-                v2_mbar_expect_tx(sBar + 8 * 3 * TS_V2_NBUF, TS_V2_TAB_BYTES);
-                v2_bulk_load(sBase + TS_V2_OFF_TAB, p.d.tables, TS_V2_TAB_BYTES, sBar + 8 * 3 * TS_V2_NBUF);
+                v2_mbar_expect_tx(sBar + TS_V2_BAR_TABLE, TS_V2_TAB_BYTES);
+                v2_bulk_load(sBase + TS_V2_OFF_TAB, p.d.tables, TS_V2_TAB_BYTES, sBar + TS_V2_BAR_TABLE);
             }
             const uint32_t per = 1u << p.pair_log2;
             const uint64_t ntick = p.ntiles >> p.pair_log2;
@@ -589,14 +602,20 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
             while (tk < ntick) {
                 const uint32_t nxt = v2_ticket_next(p.sched);
                 for (uint32_t u = 0; u < per; ++u, ++j) {
+                    // A buffer comes back half by half: the first half of the next tile is on its way while the store of
+                    // the previous tile is still reading the second half (one buffer is all the transport has while both
+                    // compute groups hold theirs, so its turn-around time is the pipeline's period).
                     const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-                    if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
                     const uint64_t tile = ((uint64_t)tk << p.pair_log2) + u;
-                    const uint32_t bar = sBar + 8 * b;
+                    const uint32_t bar = sBar + TS_V2_BAR_FULL(b);
+                    if (use > 0) v2_mbar_wait(sBar + TS_V2_BAR_FREE(b, 0), (use - 1) & 1u);
                     v2_st_tile(smraw, b, (uint32_t)tile);
-                    v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (has_diag ? 512u : 0u));
+                    v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES / 2 + (has_diag ? 512u : 0u));
                     if (has_diag) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, p.d.tile_phase + (tile << 5), 512u, bar);
-                    v2_issue_load(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, bar);
+                    v2_issue_load(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, bar, 0);
+                    if (use > 0) v2_mbar_wait(sBar + TS_V2_BAR_FREE(b, 1), (use - 1) & 1u);
+                    v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES / 2);
+                    v2_issue_load(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, bar, 1);
                 }
                 tk = nxt;
             }
@@ -605,13 +624,17 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
         } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
             for (uint64_t j = 0;; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-                v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
+                v2_mbar_wait(sBar + TS_V2_BAR_DONE(b), use & 1u);
                 const uint32_t tile = v2_ld_tile(smraw, b);
                 if (tile == TS_V2_END) break;
-                v2_issue_store(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES);
+                v2_issue_store(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, 0);
                 v2_store_commit();
+                v2_issue_store(p.g, &tmap, tile, sBase + b * TS_V2_TILE_BYTES, 1);
+                v2_store_commit();
+                v2_store_wait_read_but_one();          // the first half has been read: it can be refilled
+                v2_mbar_arrive(sBar + TS_V2_BAR_FREE(b, 0));
                 v2_store_wait_read();
-                v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
+                v2_mbar_arrive(sBar + TS_V2_BAR_FREE(b, 1));
             }
             v2_store_wait_all();
         }
@@ -621,11 +644,11 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
         const int t = threadIdx.x & (TS_TILE_THREADS - 1);
         const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
         const double scale = p.d.scale;
-        if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
+        if (has_diag) v2_mbar_wait(sBar + TS_V2_BAR_TABLE, 0u);
         if (grp >= p.ngroups) return;
         for (uint64_t j = grp;; j += p.ngroups) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-            v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
+            v2_wait_full(sBar + TS_V2_BAR_FULL(b), sBar + TS_V2_BAR_DONE(b), use);
             const bool end = (v2_ld_tile(smraw, b) == TS_V2_END);
             if (!end && !p.probe) {
                 unsigned char* buf = smraw + b * TS_V2_TILE_BYTES;
@@ -636,7 +659,7 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
                 else v2_body_H<K1, K2, -1, MODE>(buf, p.g, has_diag, scale, tp, tab, t, grp);
                 v2_fence_async_smem();                 // my shared-memory writes -> visible to the TMA store
             }
-            v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
+            v2_mbar_arrive(sBar + TS_V2_BAR_DONE(b));
             if (end) break;
         }
     }
@@ -689,8 +712,8 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
         v2_regs_dec<TS_V2_REGS_PRODUCER>();
         if (warp == 8 && (threadIdx.x & 31) == 0) {    // ---- loader
             if (has_diag) {
-                v2_mbar_expect_tx(sBar + 8 * 3 * TS_V2_NBUF, TS_V2_TAB_BYTES);
-                v2_bulk_load(sBase + TS_V2_OFF_TAB, q.d.tables, TS_V2_TAB_BYTES, sBar + 8 * 3 * TS_V2_NBUF);
+                v2_mbar_expect_tx(sBar + TS_V2_BAR_TABLE, TS_V2_TAB_BYTES);
+                v2_bulk_load(sBase + TS_V2_OFF_TAB, q.d.tables, TS_V2_TAB_BYTES, sBar + TS_V2_BAR_TABLE);
             }
             // L2 priorities: what phase 1 reads from HBM is about to be overwritten (evict first); what phases 1 and 2
             // write is read again from L2 (evict last); the third phase's reads are the last use of a line.
@@ -712,14 +735,18 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
                     }
                     v2_fence_async_all();              // the TMA engine reads what other SMs' TMA stores wrote
                 }
-                if (use > 0) v2_mbar_wait(sBar + 8 * (2 * TS_V2_NBUF + b), (use - 1) & 1u);
-                const uint32_t bar = sBar + 8 * b;
+                const uint32_t bar = sBar + TS_V2_BAR_FULL(b);
                 const bool tpl = has_diag && phase == 1;
+                const V2Geom& gj = (phase == 1) ? q.ga : q.gh;
+                const CUtensorMap* tmj = (phase == 1) ? &tmA : &tmH;
+                if (use > 0) v2_mbar_wait(sBar + TS_V2_BAR_FREE(b, 0), (use - 1) & 1u);
                 v2_st_tile(smraw, b, n);
-                v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES + (tpl ? 512u : 0u));
+                v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES / 2 + (tpl ? 512u : 0u));
                 if (tpl) v2_bulk_load(sBase + TS_V2_OFF_TP + b * 512u, q.d.tile_phase + (tile << 5), 512u, bar);
-                if (phase == 1) v2_issue_load_h(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[1]);
-                else v2_issue_load_h(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[phase]);
+                v2_issue_load_h(gj, tmj, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[phase], 0);
+                if (use > 0) v2_mbar_wait(sBar + TS_V2_BAR_FREE(b, 1), (use - 1) & 1u);
+                v2_mbar_expect_tx(bar, TS_V2_TILE_BYTES / 2);
+                v2_issue_load_h(gj, tmj, tile, sBase + b * TS_V2_TILE_BYTES, bar, pol_ld[phase], 1);
                 ++j;
                 n = nxt;
             }
@@ -729,16 +756,21 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
             const uint64_t pol_st[3] = {v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
             for (uint64_t j = 0;; ++j) {
                 const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-                v2_mbar_wait(sBar + 8 * (TS_V2_NBUF + b), use & 1u);
+                v2_mbar_wait(sBar + TS_V2_BAR_DONE(b), use & 1u);
                 const uint32_t n = v2_ld_tile(smraw, b);
                 if (n == TS_V2_END) break;
                 uint32_t phase, c; uint64_t tile;
                 job_of(n, phase, c, tile);
-                if (phase == 1) v2_issue_store_h(q.ga, &tmA, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[1]);
-                else v2_issue_store_h(q.gh, &tmH, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[phase]);
+                const V2Geom& gj = (phase == 1) ? q.ga : q.gh;
+                const CUtensorMap* tmj = (phase == 1) ? &tmA : &tmH;
+                v2_issue_store_h(gj, tmj, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[phase], 0);
                 v2_store_commit();
-                v2_store_wait_read();                  // the buffer can be refilled as soon as the store has read it
-                v2_mbar_arrive(sBar + 8 * (2 * TS_V2_NBUF + b));
+                v2_issue_store_h(gj, tmj, tile, sBase + b * TS_V2_TILE_BYTES, pol_st[phase], 1);
+                v2_store_commit();
+                v2_store_wait_read_but_one();          // a half can be refilled as soon as the store has read it
+                v2_mbar_arrive(sBar + TS_V2_BAR_FREE(b, 0));
+                v2_store_wait_read();
+                v2_mbar_arrive(sBar + TS_V2_BAR_FREE(b, 1));
                 if (phase != 2) {
                     // Publish only once the tile IS in global memory (L2).  (Not deferred to the next job: a publish
                     // that waited for this CTA's next job could wait for a job that depends on it.)
@@ -756,11 +788,11 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
         const int t = threadIdx.x & (TS_TILE_THREADS - 1);
         const double2* tab = reinterpret_cast<const double2*>(smraw + TS_V2_OFF_TAB);
         const double scale = q.d.scale;
-        if (has_diag) v2_mbar_wait(sBar + 8 * 3 * TS_V2_NBUF, 0u);
+        if (has_diag) v2_mbar_wait(sBar + TS_V2_BAR_TABLE, 0u);
         if (grp >= q.ngroups) return;
         for (uint64_t j = grp;; j += q.ngroups) {
             const uint32_t b = (uint32_t)(j % TS_V2_NBUF), use = (uint32_t)(j / TS_V2_NBUF);
-            v2_wait_full(sBar + 8 * b, sBar + 8 * (TS_V2_NBUF + b), use);
+            v2_wait_full(sBar + TS_V2_BAR_FULL(b), sBar + TS_V2_BAR_DONE(b), use);
             const uint32_t n = v2_ld_tile(smraw, b);
             const bool end = (n == TS_V2_END);
             if (!end && !q.probe) {
@@ -777,7 +809,7 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
                 else v2_body_H<KB, SW_NONE, HM, MODE>(buf, q.gh, false, 1.0, tp, tab, t, grp);
                 v2_fence_async_smem();
             }
-            v2_mbar_arrive(sBar + 8 * (TS_V2_NBUF + b));
+            v2_mbar_arrive(sBar + TS_V2_BAR_DONE(b));
             if (end) break;
         }
     }
