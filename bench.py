@@ -327,6 +327,7 @@ def run_ours(args):
     barrier()
     prof = ts.get_profile()
     ts.set_profiling(False)
+    eff_khz = ts.get_option(B.OPT_LAST_LAUNCH_KHZ) if tiled_plan(ts) else None     # the last launch of the profiled region
     norm2 = ts.norm2()
     ms = float(np.median(region_ms))
     steps_per_s = R.whole_job_steps_per_s(args.steps, world, ms)
@@ -348,10 +349,11 @@ def run_ours(args):
         barrier()
         cms = R.max_over_ranks(e0.elapsed_time(e1), dev) / args.steps
         cprof = ts.get_profile()
+        ceil_khz = ts.get_option(B.OPT_LAST_LAUNCH_KHZ)
         ts.set_option(B.OPT_PROBE, 0)
         ts.set_profiling(False)
         ceiling = {"what": "same launches, copy only (TS_OPT_PROBE=1): tile transport without the arithmetic",
-                   "ms_per_step": cms,
+                   "ms_per_step": cms, "effective_sm_mhz_last_launch": ceil_khz / 1e3,
                    "kernel_avg_ms": {k: v["ms"] / v["launches"] for k, v in cprof.items() if v["launches"] and k.startswith("tile")}}
         ts.reset_profile()
 
@@ -468,7 +470,8 @@ def run_ours(args):
            "spin_amplitude_updates_per_sec": steps_per_s * N_SWEEPS_PER_STEP * N * dim,
            "amplitude_steps_per_sec": steps_per_s * dim,
            "norm2_after": norm2, "library": B.version(), "kernel_sources_hash": kernel_sources_hash(),
-           "gpu_launches": launches, "kernels": kern, "clocks": clocks, "roofline": roofline,
+           "gpu_launches": launches, "kernels": kern, "clocks": clocks,
+           "effective_sm_mhz_last_launch": (eff_khz / 1e3) if eff_khz else None, "roofline": roofline,
            "cpu_baseline": cpu, "e2e": e2e}
     if observables is not None:
         out["observables"] = observables

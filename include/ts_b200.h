@@ -162,6 +162,8 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  *                          ts_evolve call of >= 4 steps captures the launches of one step into a CUDA graph and replays it;
  *                          0: every launch goes to the stream one by one.  Off while profiling is on.
  *   TS_OPT_GRAPH_MAX_N     see above (12..33).   TS_OPT_GRAPH_REPLAYS (read-only): graph replays so far
+ *   TS_OPT_LAST_LAUNCH_KHZ (read-only, synchronises): the SM clock the last persistent tile launch really ran at, in kHz: SM
+ *                          cycles / wall nanoseconds between the start and the last ticket of CTA 0's loader
  *   TS_OPT_L2_PROMOTION    tensor-map L2 promotion of the high groups: 0 none (default), 1: 128 B, 2: 256 B
  *   TS_OPT_SMALL           1 (default): under TS_PLAN_AUTO, N <= 12 runs a whole ts_evolve call as one single-CTA launch
  *                          (state in shared memory; small systems are latency-bound); 0: tiled / naive plans
@@ -182,7 +184,8 @@ int ts_set_plan_groups(ts_ctx* ctx, int n_high, const int* high_bits);
  * Errors: TS_ERR_ARG (unknown key, value out of range). */
 enum { TS_OPT_KERNEL = 0, TS_OPT_CHUNK = 1, TS_OPT_CHUNK_MAX_LOG2 = 2, TS_OPT_L2_PROMOTION = 3, TS_OPT_SMALL = 4,
        TS_OPT_DIAG_SOURCE = 5, TS_OPT_MAX_CTAS = 6, TS_OPT_L2_HINTS = 7, TS_OPT_PAIR = 8, TS_OPT_PROBE = 9,
-       TS_OPT_CHUNK_MIN_LOG2 = 10, TS_OPT_GRAPH = 11, TS_OPT_GRAPH_MAX_N = 12, TS_OPT_GRAPH_REPLAYS = 13 };
+       TS_OPT_CHUNK_MIN_LOG2 = 10, TS_OPT_GRAPH = 11, TS_OPT_GRAPH_MAX_N = 12, TS_OPT_GRAPH_REPLAYS = 13,
+       TS_OPT_LAST_LAUNCH_KHZ = 14 };
 int ts_set_option(ts_ctx* ctx, int key, int value);
 int ts_get_option(ts_ctx* ctx, int key, int* value);
 

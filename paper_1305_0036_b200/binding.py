@@ -18,7 +18,7 @@ TS_OK, TS_ERR_ARG, TS_ERR_NOMEM, TS_ERR_CUDA, TS_ERR_NOSTATE = 0, -1, -2, -3, -4
 X, Y, Z = 0, 1, 2
 HOST, DEVICE = 0, 1
 PLAN_AUTO, PLAN_NAIVE, PLAN_TILED = 0, 1, 2
-OPT_KERNEL, OPT_CHUNK, OPT_CHUNK_MAX_LOG2, OPT_L2_PROMOTION, OPT_SMALL, OPT_DIAG_SOURCE, OPT_MAX_CTAS, OPT_L2_HINTS, OPT_PAIR, OPT_PROBE, OPT_CHUNK_MIN_LOG2, OPT_GRAPH, OPT_GRAPH_MAX_N, OPT_GRAPH_REPLAYS = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13
+OPT_KERNEL, OPT_CHUNK, OPT_CHUNK_MAX_LOG2, OPT_L2_PROMOTION, OPT_SMALL, OPT_DIAG_SOURCE, OPT_MAX_CTAS, OPT_L2_HINTS, OPT_PAIR, OPT_PROBE, OPT_CHUNK_MIN_LOG2, OPT_GRAPH, OPT_GRAPH_MAX_N, OPT_GRAPH_REPLAYS, OPT_LAST_LAUNCH_KHZ = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14
 KC_NAMES = ("tile_fused", "tile_single", "naive_rot", "naive_diag", "reduce", "setup", "tile_chunk3", "small")
 KC_COUNT = len(KC_NAMES)
 

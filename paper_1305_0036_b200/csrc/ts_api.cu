@@ -437,8 +437,8 @@ int ts_create(ts_ctx** out, int N, const double* h, const double* J)
     if (e == cudaSuccess) e = cudaMalloc(&c->d_Jeff, sizeof(c->Jeff));
     if (e == cudaSuccess) e = cudaMemcpy(c->d_h, c->h, sizeof(c->h), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(c->d_Jeff, c->Jeff, sizeof(c->Jeff), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, 2 * sizeof(unsigned int));
-    if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 2 * sizeof(unsigned int));   // kernels leave it at zero
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, 8 * sizeof(unsigned int));     // [0..1] tickets, [2..5] clock probe
+    if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 8 * sizeof(unsigned int));   // kernels leave the tickets at zero
     if (e == cudaSuccess) e = ts_tile_init();
     if (e == cudaSuccess) e = ts_small_init();
     if (e != cudaSuccess) { cudaGetLastError(); ts_destroy(c); return cuda_status(e); }
@@ -614,6 +614,14 @@ int ts_get_option(ts_ctx* c, int key, int* value)
     case TS_OPT_PAIR: *value = c->opt_pair; break;
     case TS_OPT_GRAPH: *value = c->opt_graph; break;
     case TS_OPT_GRAPH_MAX_N: *value = c->opt_graph_max_n; break;
+    case TS_OPT_LAST_LAUNCH_KHZ: {
+        // effective SM clock of the last persistent tile launch: cycles / nanoseconds seen by CTA 0's loader (synchronises)
+        unsigned long long v[2] = {0, 0};
+        if (cudaStreamSynchronize(c->stream) != cudaSuccess ||
+            cudaMemcpy(v, c->d_sched + 2, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return TS_ERR_CUDA; }
+        *value = v[1] ? (int)((double)v[0] / (double)v[1] * 1e6) : 0;
+        break;
+    }
     case TS_OPT_GRAPH_REPLAYS: *value = (int)(c->graph_replays > 0x7fffffff ? 0x7fffffff : c->graph_replays); break;
     case TS_OPT_CHUNK_MIN_LOG2: *value = c->opt_chunk_min_log2; break;
     case TS_OPT_PROBE: *value = c->opt_probe; break;

@@ -545,6 +545,22 @@ __device__ __forceinline__ void v2_ticket_finish(unsigned int* sched)
         __threadfence();
     }
 }
+// Effective SM clock of a launch: CTA 0's loader reads the SM cycle counter and the global nanosecond timer when it starts
+// and when it has drawn its last ticket, and leaves both differences in sched[2..5].  Under a power cap the clock a
+// sampling tool reports and the cycles the SMs really get can differ; this is the latter (TS_OPT_LAST_LAUNCH_KHZ).
+__device__ __forceinline__ void v2_clock_read(unsigned long long& cyc, unsigned long long& ns)
+{
+    asm volatile("mov.u64 %0, %%clock64;" : "=l"(cyc));
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
+}
+__device__ __forceinline__ void v2_clock_leave(unsigned int* sched, const unsigned long long c0, const unsigned long long t0)
+{
+    unsigned long long c1, t1;
+    v2_clock_read(c1, t1);
+    unsigned long long* out = reinterpret_cast<unsigned long long*>(sched + 2);
+    out[0] = c1 - c0;
+    out[1] = t1 - t0;
+}
 __device__ __forceinline__ uint32_t v2_ld_tile(const unsigned char* smraw, uint32_t b)
 {
     return *reinterpret_cast<const volatile uint32_t*>(smraw + TS_V2_OFF_TILE + 4u * b);
@@ -598,6 +614,8 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
             const uint32_t per = 1u << p.pair_log2;
             const uint64_t ntick = p.ntiles >> p.pair_log2;
             uint64_t j = 0;
+            unsigned long long clk0 = 0, ns0 = 0;
+            if (blockIdx.x == 0) v2_clock_read(clk0, ns0);
             uint32_t tk = v2_ticket_next(p.sched);
             while (tk < ntick) {
                 const uint32_t nxt = v2_ticket_next(p.sched);
@@ -620,6 +638,7 @@ k_tile_v2(const __grid_constant__ V2Pass p, const __grid_constant__ CUtensorMap 
                 tk = nxt;
             }
             v2_push_end(smraw, sBar, j);
+            if (blockIdx.x == 0) v2_clock_leave(p.sched, clk0, ns0);
             v2_ticket_finish(p.sched);
         } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
             for (uint64_t j = 0;; ++j) {
@@ -720,6 +739,8 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
             const uint64_t pol_ld[3] = {v2_policy(q.l2_hints ? 1 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
             uint32_t ok_key = 0xffffffffu;             // (phase, chunk) whose dependency was last seen satisfied
             uint64_t j = 0;
+            unsigned long long clk0 = 0, ns0 = 0;
+            if (blockIdx.x == 0) v2_clock_read(clk0, ns0);
             uint32_t n = v2_ticket_next(q.sched);
             while (n < total) {
                 const uint32_t nxt = v2_ticket_next(q.sched);
@@ -751,6 +772,7 @@ k_chunk_v2(const __grid_constant__ V2Chunk q, const __grid_constant__ CUtensorMa
                 n = nxt;
             }
             v2_push_end(smraw, sBar, j);
+            if (blockIdx.x == 0) v2_clock_leave(q.sched, clk0, ns0);
             v2_ticket_finish(q.sched);
         } else if (warp == 9 && (threadIdx.x & 31) == 0) {   // ---- storer
             const uint64_t pol_st[3] = {v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 2 : 0), v2_policy(q.l2_hints ? 1 : 0)};
