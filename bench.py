@@ -450,7 +450,7 @@ def run_ours(args):
                 "note": ("frac = HBM bytes of the dominant launch / its time / peak.  The L2-blocked launch makes three tile "
                          "passes per HBM round trip and L2-resident passes move at most ~7.7 TB/s on this part, so its HBM "
                          "fraction cannot reach 1; transport_ceiling is the measured bound of the same launches without "
-                         "arithmetic, and the run is power-capped (clocks.reasons)") if hbm_resident
+                         "arithmetic; clocks.reasons says whether the run hit the power cap") if hbm_resident
                         else "state fits in L2: absolute steps/s is the figure, not an HBM fraction"}
     cpu = None
     if not args.no_cpu:

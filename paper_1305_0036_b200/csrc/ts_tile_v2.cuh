@@ -341,6 +341,21 @@ __device__ __forceinline__ void v2_apply_diag(const double2* RR, const double2 b
     }
 }
 
+// Measurement builds without arithmetic: swap neighbouring registers after every shared-memory load, so that what is stored
+// differs from what was loaded and the compiler cannot drop the exchange as a load followed by a store of the same value
+// (it did: an earlier "exchanges only" build ran with 1 % shared-memory traffic).
+template <bool ON>
+__device__ __forceinline__ void v2_probe_touch(double (&re)[32], double (&im)[32])
+{
+    if (!ON) return;
+#pragma unroll
+    for (int r = 0; r < 32; r += 2) {
+        const double a = re[r], b = im[r];
+        re[r] = re[r + 1]; im[r] = im[r + 1];
+        re[r + 1] = a; im[r + 1] = b;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ tile bodies
 // The tile is in `buf` (landed by TMA); on return the finished tile is in `buf` again, in the same slots.
 // diag: apply the diagonal; tp: this tile's phase record; tab: the launch's thread tables (both in shared memory).
@@ -358,11 +373,13 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, c
     double re[32], im[32];
     if (K1 != SW_NONE) {
         L1::load(buf, o1, re, im);
+        v2_probe_touch<!AR>(re, im);
         if (AR) bfly_regs<K1, 31>(re, im, 0u);         // f 3,4,5,10,11
         if (EX) {
             L1::store(buf, o1, re, im);
             v2_group_sync(grp);
             L2::load(buf, o2, re, im);
+            v2_probe_touch<!AR>(re, im);
         }
         if (AR) bfly_regs<K1, 31>(re, im, 0u);         // f 0,1,2,8,9
         if (EX) {
@@ -371,6 +388,7 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, c
         }
     }
     if (EX || K1 == SW_NONE) L2S::load(buf, o2s, re, im);
+    v2_probe_touch<!AR>(re, im);
     if (AR) bfly_regs<K1, 24>(re, im, 0u);             // f 6,7
     if (diag && AR) {
         double2 base, w[5];
@@ -383,12 +401,14 @@ __device__ __forceinline__ void v2_body_A(unsigned char* buf, const bool diag, c
             L2S::store(buf, o2s, re, im);
             v2_group_sync(grp);
             L1::load(buf, o1, re, im);
+            v2_probe_touch<!AR>(re, im);
         }
         if (AR) bfly_regs<K2, 31>(re, im, 0u);         // f 3,4,5,10,11
         if (EX) {
             L1::store(buf, o1, re, im);                // A1 -> A1'
             __syncwarp();
             L1S::load(buf, o1s, re, im);
+            v2_probe_touch<!AR>(re, im);
         }
         if (AR) bfly_regs<K2, 24>(re, im, 0u);         // f 8,9
         if (EX) L1S::store(buf, o1s, re, im);
@@ -422,11 +442,13 @@ __device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, c
     const bool two = EX && (CT ? (M > 5) : (g.two_stage != 0));
     double re[32], im[32];
     L1::load(buf, o1, re, im);
+    v2_probe_touch<!AR>(re, im);
     if (AR) bfly_regs<K1, MK1>(re, im, g.mask1);
     if (two) {
         L1::store(buf, o1, re, im);
         v2_group_sync(grp);
         L2::load(buf, o2, re, im);
+        v2_probe_touch<!AR>(re, im);
     }
     if (AR && (two || !EX)) bfly_regs<K1, MK2>(re, im, g.mask2);
     if (diag && AR) {
@@ -440,6 +462,7 @@ __device__ __forceinline__ void v2_body_H(unsigned char* buf, const V2Geom& g, c
             L2::store(buf, o2, re, im);
             v2_group_sync(grp);
             L1::load(buf, o1, re, im);
+            v2_probe_touch<!AR>(re, im);
         }
         if (AR) bfly_regs<K2, MK1>(re, im, g.mask1);
         L1::store(buf, o1, re, im);
