@@ -434,3 +434,15 @@ def test_evolve_observe_graph_replay_matches_launch_by_launch(B):
     for k in range(steps):
         O.evolve(psi, N, w.h, w.J, w.tau, 1, 4, True)
         assert np.max(np.abs(traces[0][k] - O.expect_all(psi, N, O.Z))) <= OBS_TOL
+
+
+def test_effective_clock_probe(B):
+    """TS_OPT_LAST_LAUNCH_KHZ: SM cycles per wall nanosecond as seen by CTA 0's loader of the last persistent launch."""
+    N = 24
+    w = W.generic(N, seed=77, tau=0.01, n_steps=1)
+    ts = B.TrotterSuzuki(N, w.h, w.J)
+    ts.set_random_phase_state(0, seed=1)
+    ts.evolve(w.tau, 2, 4)
+    khz = ts.get_option(B.OPT_LAST_LAUNCH_KHZ)
+    assert 300_000 < khz < 3_000_000, khz
+    ts.close()
